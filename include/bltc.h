@@ -1,0 +1,187 @@
+/*
+ * bltc.h -- C ABI of libbltc: the discrete modified-Helmholtz (Yukawa) convolution of
+ * treecode-accelerated Green Iteration (arXiv 2003.01833) on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed, for every orbital o and target point x_i (Eq. (18) discretised
+ * as PAPER.md:371 Eq. (32), with the singularity subtraction of PAPER.md:204-208 Eq. (20)-(21)):
+ *
+ *   subtract_singularity = 1:
+ *     out[o][i] = -2 * ( sum_{j : r_ij != 0} G_k(r_ij) w_j (f[o][j] - f[o][i])  +  f[o][i] / k_o^2 )
+ *   subtract_singularity = 0:
+ *     out[o][i] = -2 *   sum_{j : r_ij != 0} G_k(r_ij) w_j  f[o][j]
+ *
+ *   G_k(r) = exp(-k r) / (4 pi r),   k_o = sqrt(-2 eps_o) > 0,   r_ij = |x_i - y_j|.
+ *
+ * "The singular r' = r term in the quadrature sums is skipped": a term is skipped
+ * iff r_ij == 0 exactly.  direct_convolve evaluates the sum as written (O(M N)); bltc_convolve
+ * evaluates it with the barycentric Lagrange treecode of PAPER.md:361-462 (Section 6, Algorithm 3):
+ * source-cluster tree, target batches and MAC interaction lists built once per mesh by bltc_create,
+ * proxy charges on tensor Chebyshev grids (Eq. (35) right, (37)-(39)), batch-cluster far field
+ * (Eq. (35) left) and batch-leaf direct near field (Eq. (34)).
+ *
+ * Conventions
+ *   - All floating point is IEEE double.  Coordinates are SoA: double[3][N] = x-row, y-row, z-row.
+ *   - Every data pointer may be a DEVICE pointer or a HOST pointer; the library asks
+ *     cudaPointerGetAttributes.  Host buffers are staged through device memory inside the call
+ *     (copies are enqueued on `stream`).  k is always a HOST array.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls that
+ *     take a stream only ENQUEUE work and return without synchronising, except when `out` is a
+ *     host pointer: then the call returns after the stream has been synchronised.
+ *   - The library copies what it needs: inputs of bltc_create may be freed after it returns;
+ *     f/out of a convolve call must stay valid until the stream has executed the call.
+ *   - Return value: 0 on success, a negative bltc_status otherwise; bltc_last_error() gives a
+ *     thread-local message.  No exceptions, no exit(), no global state; handles are independent.
+ *     A handle must not be used by two threads at once.
+ *   - There is no CPU fallback: every compute entry point fails with BLTC_ECUDA / BLTC_ENODEVICE
+ *     if no CUDA device is usable.
+ *   - Limits: 1 <= N <= 2e9 (int32 indices), 1 <= interp_degree <= 20, 0 <= theta < 1,
+ *     1 <= n_orb, k_o > 0 and k_o * (domain diameter) < 2^30.
+ */
+#ifndef BLTC_H_
+#define BLTC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bltc_plan_s* bltc_handle;   /* opaque, owned by the library */
+typedef void* bltc_stream;                 /* cudaStream_t */
+
+typedef enum bltc_status {
+    BLTC_OK = 0,
+    BLTC_EINVAL = -1,      /* bad argument (message says which) */
+    BLTC_ENOMEM = -2,      /* host or device allocation failed */
+    BLTC_ECUDA = -3,       /* a CUDA call failed (message carries cudaGetErrorString) */
+    BLTC_ENODEVICE = -4    /* handle has no device state (bltc_create_host_plan) */
+} bltc_status;
+
+/* Counters of a plan (step a0).  "evals" = kernel evaluations per orbital per convolution. */
+typedef struct bltc_stats {
+    int64_t n_points;          /* N */
+    int64_t n_clusters;        /* source clusters in the tree */
+    int64_t n_leaves;          /* leaf clusters */
+    int64_t n_batches;         /* target batches */
+    int64_t n_far;             /* batch-cluster far interactions, total (Eq. (35)) */
+    int64_t n_near;            /* batch-cluster direct interactions, total (Eq. (34)) */
+    int64_t far_evals;         /* sum over far interactions of targets * (n+1)^3 */
+    int64_t near_evals;        /* sum over near interactions of targets * N_S */
+    int64_t n_proxy_clusters;  /* clusters that carry proxy charges */
+    int64_t upward_pairs;      /* sum over those clusters of N_S */
+    int64_t n_far_items;       /* CTAs launched by the far-field kernel (R = 2 tiling) */
+    int64_t n_near_items;      /* CTAs launched by the near-field kernel (R = 2 tiling) */
+    int64_t partial_len;       /* doubles of partial-sum scratch per orbital */
+    int32_t shared_batches;    /* 1: batches are the source leaves */
+    int32_t interp_degree;
+    double  theta;
+    double  build_ms;          /* host wall-clock of tree + lists + work decomposition */
+    double  upload_ms;         /* host wall-clock of device upload + f-independent proxy weights */
+} bltc_stats;
+
+/* Phases of one bltc_convolve, for bltc_get_phase_ms (device times, CUDA events on `stream`). */
+enum { BLTC_PHASE_GATHER = 0, BLTC_PHASE_UPWARD = 1, BLTC_PHASE_FAR = 2, BLTC_PHASE_NEAR = 3,
+       BLTC_PHASE_EPILOGUE = 4, BLTC_NUM_PHASES = 5 };
+
+/*
+ * bltc_create: Algorithm 3 line 1 plus everything that does not depend on f or k.
+ *   targets  double[3][N] SoA, or NULL / == sources when the targets are the sources (the TAGI case:
+ *            "the target particles and source particles correspond to the same set").
+ *   sources  double[3][N] SoA.        weights  double[N] quadrature weights w_j.
+ *   theta, interp_degree: MAC parameter and degree n of Eq. (36).
+ *   batch_size N_B, leaf_size N_L: PAPER.md:378,428.  If N_B == N_L and targets are the sources the
+ *   batches are the leaf clusters.
+ * Builds the tree, batches, lists on the host, uploads tree-ordered data and computes the proxy
+ * weights of w (what_k).  Synchronous.  *h is set only on success.
+ */
+int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                int64_t N, double theta, int interp_degree, int batch_size, int leaf_size);
+
+/* Same plan, host part only (no CUDA call is made): for structural inspection through
+ * bltc_get_stats / bltc_export_plan.  weights may be NULL.  bltc_convolve on such a handle
+ * returns BLTC_ENODEVICE.  coordinates must be HOST pointers. */
+int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* sources,
+                          const double* weights, int64_t N, double theta, int interp_degree,
+                          int batch_size, int leaf_size);
+
+/*
+ * bltc_convolve: Algorithm 3 lines 2-3 + Eq. (18),(20),(21), all orbitals.
+ *   k    HOST double[n_orb], k_o > 0 (one per orbital: each wavefunction has its own eps).
+ *   f    double[n_orb][N], caller's original point order: f = V_eff * psi at the quadrature points.
+ *   out  double[n_orb][N], caller's original point order.
+ *   subtract_singularity = 1 requires that the plan's targets are its sources.
+ * Steps (all on `stream`): gather to tree order; upward pass (proxy charges fhat_k of f*w);
+ * far-field kernel; near-field kernel; epilogue (-2 (far + near + f_i/k^2), scatter).
+ */
+int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
+                  int subtract_singularity, bltc_stream stream);
+
+/*
+ * direct_convolve: the definition, O(M N), no plan (Eq. (32); the "ds" column of
+ * PAPER.md:482-490 Table 4).  M targets against N sources.
+ *   targets double[3][M], f_targets double[n_orb][M] (may be NULL iff subtract_singularity == 0),
+ *   sources double[3][N], weights double[N], f_sources double[n_orb][N], k HOST double[n_orb],
+ *   out double[n_orb][M].
+ */
+int direct_convolve(const double* targets, const double* f_targets, int64_t M,
+                    const double* sources, const double* weights, const double* f_sources, int64_t N,
+                    const double* k, int n_orb, double* out, int subtract_singularity,
+                    bltc_stream stream);
+
+int bltc_destroy(bltc_handle h);
+
+int bltc_get_stats(bltc_handle h, bltc_stats* s);
+
+/*
+ * bltc_export_plan: copy the plan's structure into caller-provided HOST buffers (any may be NULL),
+ * for comparison with an independently built tree.  Sizes come from bltc_get_stats.
+ *   src_perm[N], tgt_perm[N]        tree order -> caller index (sources, targets)
+ *   cl_begin/cl_end[n_clusters]     particle range of each cluster in source tree order (DFS pre-order ids)
+ *   cl_lo/cl_hi[n_clusters][3]      minimal bounding boxes
+ *   cl_parent/cl_nchild[n_clusters]
+ *   b_begin/b_end[n_batches]        target range of each batch in target tree order
+ *   far_ptr/near_ptr[n_batches+1], far_idx[n_far], near_idx[n_near]   CSR lists of cluster ids,
+ *                                   in the traversal order of Algorithm 3
+ */
+int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
+                     int64_t* cl_begin, int64_t* cl_end, double* cl_lo, double* cl_hi,
+                     int32_t* cl_parent, int32_t* cl_nchild, int64_t* b_begin, int64_t* b_end,
+                     int64_t* far_ptr, int32_t* far_idx, int64_t* near_ptr, int32_t* near_idx);
+
+/*
+ * bltc_export_proxy: after a bltc_convolve has completed on the device, copy the Chebyshev grids and
+ * proxy charges of the LAST orbital group to HOST buffers (any may be NULL):
+ *   proxy_cluster[n_proxy_clusters]          cluster id of each proxy slot
+ *   nodes[n_proxy_clusters][3][n+1]          Eq. (37) mapped to the cluster box
+ *   what[n_proxy_clusters][(n+1)^3]          proxy weights of w
+ *   fhat[n_proxy_clusters][(n+1)^3][ot]      proxy charges of f*w for the `*ot` orbitals of that group
+ * Synchronises the device.
+ */
+int bltc_export_proxy(bltc_handle h, int32_t* proxy_cluster, double* nodes, double* what,
+                      double* fhat, int32_t* ot);
+
+/* Per-phase device timing.  enable = 1: every later bltc_convolve records CUDA events on its stream
+ * around each phase.  bltc_get_phase_ms synchronises on the last recorded event and returns the
+ * milliseconds of each phase of the most recent convolve, summed over its orbital groups. */
+int bltc_set_profiling(bltc_handle h, int enable);
+int bltc_get_phase_ms(bltc_handle h, float ms[BLTC_NUM_PHASES]);
+
+/* Device time (ms, CUDA events) of the pair kernel inside the most recent direct_convolve that was
+ * called with profiling on (bltc_direct_set_profiling(1)); synchronises on its last event. */
+int bltc_direct_set_profiling(int enable);
+int bltc_direct_get_kernel_ms(float* ms);
+
+/*
+ * bltc_probe_fp64: measurement utility for the roofline denominator.  Runs a kernel of dependent-
+ * chain-free DFMA instructions on every SM for about `iters` x 4096 DFMAs per thread and reports the
+ * achieved FP64 rate in TFLOP/s (2 flops per DFMA) in *tflops, timed with CUDA events on `stream`.
+ */
+int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream);
+
+const char* bltc_last_error(void);
+const char* bltc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLTC_H_ */

@@ -1,0 +1,248 @@
+"""Thin ctypes binding of libbltc (include/bltc.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; nothing is computed here.
+Arguments may be torch tensors (CUDA or CPU, float64, contiguous) or numpy float64 arrays; the
+library itself decides host vs device from the raw pointer.  There is no CPU fallback: if
+libbltc.so cannot be built/loaded, importing the entry points raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+BLTC_OK, BLTC_EINVAL, BLTC_ENOMEM, BLTC_ECUDA, BLTC_ENODEVICE = 0, -1, -2, -3, -4
+PHASES = ("gather", "upward", "far", "near", "epilogue")
+
+_dp = C.POINTER(C.c_double)
+_i64p = C.POINTER(C.c_int64)
+_i32p = C.POINTER(C.c_int32)
+
+
+class BltcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libbltc error {code}: {msg}")
+        self.code = code
+
+
+class bltc_stats(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in (
+        "n_points", "n_clusters", "n_leaves", "n_batches", "n_far", "n_near", "far_evals", "near_evals",
+        "n_proxy_clusters", "upward_pairs", "n_far_items", "n_near_items", "partial_len")] + [
+        ("shared_batches", C.c_int32), ("interp_degree", C.c_int32),
+        ("theta", C.c_double), ("build_ms", C.c_double), ("upload_ms", C.c_double)]
+
+
+EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_convolve", "direct_convolve", "bltc_destroy",
+            "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
+            "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
+            "bltc_probe_fp64", "bltc_last_error", "bltc_version")
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) paper_2003_01833_b200/libbltc.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp = C.c_void_p
+    L.bltc_last_error.restype = C.c_char_p
+    L.bltc_version.restype = C.c_char_p
+    L.bltc_create.argtypes = [C.POINTER(vp), vp, vp, vp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_int]
+    L.bltc_create_host_plan.argtypes = L.bltc_create.argtypes
+    L.bltc_convolve.argtypes = [vp, _dp, vp, C.c_int, vp, C.c_int, vp]
+    L.direct_convolve.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, _dp, C.c_int, vp, C.c_int, vp]
+    L.bltc_destroy.argtypes = [vp]
+    L.bltc_get_stats.argtypes = [vp, C.POINTER(bltc_stats)]
+    L.bltc_export_plan.argtypes = [vp, _i64p, _i64p, _i64p, _i64p, _dp, _dp, _i32p, _i32p, _i64p, _i64p,
+                                   _i64p, _i32p, _i64p, _i32p]
+    L.bltc_export_proxy.argtypes = [vp, _i32p, _dp, _dp, _dp, _i32p]
+    L.bltc_set_profiling.argtypes = [vp, C.c_int]
+    L.bltc_get_phase_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.bltc_direct_set_profiling.argtypes = [C.c_int]
+    L.bltc_direct_get_kernel_ms.argtypes = [C.POINTER(C.c_float)]
+    L.bltc_probe_fp64.argtypes = [C.c_int, _dp, vp]
+    for name in EXPORTED:
+        f = getattr(L, name)
+        if name not in ("bltc_last_error", "bltc_version"):
+            f.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        raise BltcError(rc, lib().bltc_last_error().decode())
+
+
+def _ptr(a, what, allow_none=False):
+    """Raw address of a float64 contiguous torch tensor / numpy array (keeps no reference)."""
+    if a is None:
+        if allow_none:
+            return None
+        raise ValueError(f"{what} must not be None")
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"]:
+            raise ValueError(f"{what}: need a C-contiguous float64 array")
+        return a.ctypes.data
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.dtype != torch.float64 or not a.is_contiguous():
+            raise ValueError(f"{what}: need a contiguous float64 tensor")
+        return a.data_ptr()
+    raise TypeError(f"{what}: expected numpy array or torch tensor")
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return torch.cuda.current_stream().cuda_stream
+        return None
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _karray(k, n_orb):
+    k = np.ascontiguousarray(np.atleast_1d(np.asarray(k, dtype=np.float64)))
+    if k.shape != (n_orb,):
+        raise ValueError(f"k must have shape ({n_orb},)")
+    return k
+
+
+class Plan:
+    """Handle returned by bltc_create / bltc_create_host_plan."""
+
+    def __init__(self, handle, N):
+        self._h = handle
+        self.N = N
+
+    def destroy(self):
+        if self._h:
+            lib().bltc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def _create(fn, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
+    h = C.c_void_p()
+    _check(fn(C.byref(h), _ptr(targets, "targets", True), _ptr(sources, "sources"),
+              _ptr(weights, "weights", True), int(N), float(theta), int(interp_degree),
+              int(batch_size), int(leaf_size)))
+    return Plan(h, int(N))
+
+
+def bltc_create(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
+    """include/bltc.h bltc_create.  targets may be None (targets are the sources)."""
+    return _create(lib().bltc_create, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size)
+
+
+def bltc_create_host_plan(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
+    return _create(lib().bltc_create_host_plan, targets, sources, weights, N, theta, interp_degree,
+                   batch_size, leaf_size)
+
+
+def bltc_convolve(plan, k, f, n_orb, out, subtract_singularity=True, stream=None):
+    """include/bltc.h bltc_convolve.  f, out: [n_orb][N] device or host buffers."""
+    kk = _karray(k, n_orb)
+    _check(lib().bltc_convolve(plan._h, kk.ctypes.data_as(_dp), _ptr(f, "f"), int(n_orb), _ptr(out, "out"),
+                               int(bool(subtract_singularity)), _stream_ptr(stream)))
+    return out
+
+
+def direct_convolve(targets, f_targets, M, sources, weights, f_sources, N, k, n_orb, out,
+                    subtract_singularity=True, stream=None):
+    """include/bltc.h direct_convolve."""
+    kk = _karray(k, n_orb)
+    _check(lib().direct_convolve(_ptr(targets, "targets"), _ptr(f_targets, "f_targets", True), int(M),
+                                 _ptr(sources, "sources"), _ptr(weights, "weights"),
+                                 _ptr(f_sources, "f_sources"), int(N), kk.ctypes.data_as(_dp), int(n_orb),
+                                 _ptr(out, "out"), int(bool(subtract_singularity)), _stream_ptr(stream)))
+    return out
+
+
+def bltc_destroy(plan):
+    plan.destroy()
+
+
+def bltc_get_stats(plan):
+    s = bltc_stats()
+    _check(lib().bltc_get_stats(plan._h, C.byref(s)))
+    return {n: getattr(s, n) for n, _ in bltc_stats._fields_}
+
+
+def bltc_export_plan(plan):
+    st = bltc_get_stats(plan)
+    nc, nb, N = st["n_clusters"], st["n_batches"], st["n_points"]
+    o = dict(
+        src_perm=np.empty(N, np.int64), tgt_perm=np.empty(N, np.int64),
+        cl_begin=np.empty(nc, np.int64), cl_end=np.empty(nc, np.int64),
+        cl_lo=np.empty((nc, 3)), cl_hi=np.empty((nc, 3)),
+        cl_parent=np.empty(nc, np.int32), cl_nchild=np.empty(nc, np.int32),
+        b_begin=np.empty(nb, np.int64), b_end=np.empty(nb, np.int64),
+        far_ptr=np.empty(nb + 1, np.int64), far_idx=np.empty(st["n_far"], np.int32),
+        near_ptr=np.empty(nb + 1, np.int64), near_idx=np.empty(st["n_near"], np.int32))
+    p64 = lambda a: a.ctypes.data_as(_i64p)
+    p32 = lambda a: a.ctypes.data_as(_i32p)
+    pd = lambda a: a.ctypes.data_as(_dp)
+    _check(lib().bltc_export_plan(
+        plan._h, p64(o["src_perm"]), p64(o["tgt_perm"]), p64(o["cl_begin"]), p64(o["cl_end"]),
+        pd(o["cl_lo"]), pd(o["cl_hi"]), p32(o["cl_parent"]), p32(o["cl_nchild"]),
+        p64(o["b_begin"]), p64(o["b_end"]), p64(o["far_ptr"]), p32(o["far_idx"]),
+        p64(o["near_ptr"]), p32(o["near_idx"])))
+    return o
+
+
+def bltc_export_proxy(plan):
+    st = bltc_get_stats(plan)
+    ns, n1 = st["n_proxy_clusters"], st["interp_degree"] + 1
+    P = n1 ** 3
+    cl = np.empty(ns, np.int32); nodes = np.empty((ns, 3, n1)); what = np.empty((ns, P))
+    fhat = np.zeros((ns, P, 4)); ot = C.c_int32(0)
+    _check(lib().bltc_export_proxy(plan._h, cl.ctypes.data_as(_i32p), nodes.ctypes.data_as(_dp),
+                                   what.ctypes.data_as(_dp), fhat.ctypes.data_as(_dp), C.byref(ot)))
+    o = ot.value
+    fh = fhat.reshape(-1)[: ns * P * o].reshape(ns, P, o) if o else np.zeros((ns, P, 0))
+    return dict(cluster=cl, nodes=nodes, what=what, fhat=fh)
+
+
+def bltc_set_profiling(plan, enable=True):
+    _check(lib().bltc_set_profiling(plan._h, int(bool(enable))))
+
+
+def bltc_get_phase_ms(plan):
+    ms = (C.c_float * len(PHASES))()
+    _check(lib().bltc_get_phase_ms(plan._h, ms))
+    return dict(zip(PHASES, [float(v) for v in ms]))
+
+
+def bltc_direct_set_profiling(enable=True):
+    _check(lib().bltc_direct_set_profiling(int(bool(enable))))
+
+
+def bltc_direct_get_kernel_ms():
+    ms = C.c_float(0)
+    _check(lib().bltc_direct_get_kernel_ms(C.byref(ms)))
+    return float(ms.value)
+
+
+def bltc_probe_fp64(iters=64, stream=None):
+    t = C.c_double(0)
+    _check(lib().bltc_probe_fp64(int(iters), C.byref(t), _stream_ptr(stream)))
+    return float(t.value)
+
+
+def bltc_version():
+    return lib().bltc_version().decode()

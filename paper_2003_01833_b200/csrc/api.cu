@@ -1,0 +1,600 @@
+// api.cu -- the C ABI of libbltc (include/bltc.h): argument checking, host<->device staging,
+// device state of a plan, and the launch sequence of one convolution.  No arithmetic of the
+// method lives here; it is all in kernels.cu (device) and plan_host.cpp (tree and lists).
+#include <cuda_runtime.h>
+
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <stdexcept>
+#include <string>
+#include <vector>
+
+#include "../../include/bltc.h"
+#include "kernels.cuh"
+#include "plan_host.hpp"
+
+using namespace bltc;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+
+#define BLTC_CUDA(call)                                                                        \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess) {                                                              \
+            cudaGetLastError();                                                                \
+            return fail(e__ == cudaErrorMemoryAllocation ? BLTC_ENOMEM : BLTC_ECUDA,           \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                  \
+        }                                                                                      \
+    } while (0)
+
+// true if the device can dereference p (device or managed memory)
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <typename T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t n = 0;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t ensure(size_t count) {
+        if (count <= n && p) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; n = 0; }
+        if (count == 0) count = 1;
+        cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+        if (e == cudaSuccess) n = count;
+        return e;
+    }
+    cudaError_t upload(const std::vector<T>& v) {
+        cudaError_t e = ensure(v.size());
+        if (e != cudaSuccess || v.empty()) return e;
+        return cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+};
+
+// Stream-ordered temporary (direct_convolve and host staging): freed on the stream.
+struct TempBuf {
+    void* p = nullptr;
+    cudaStream_t st = nullptr;
+    ~TempBuf() { if (p) cudaFreeAsync(p, st); }
+    cudaError_t alloc(size_t bytes, cudaStream_t s) {
+        st = s;
+        return cudaMallocAsync(&p, bytes ? bytes : 1, s);
+    }
+    template <typename T> T* as() const { return static_cast<T*>(p); }
+};
+
+// Returns a device-readable view of `src` (count doubles): src itself, or a staged copy.
+cudaError_t stage_in(const double* src, size_t count, TempBuf& tmp, cudaStream_t st, const double** dev) {
+    if (!src) { *dev = nullptr; return cudaSuccess; }
+    if (is_device_ptr(src)) { *dev = src; return cudaSuccess; }
+    cudaError_t e = tmp.alloc(count * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(tmp.p, src, count * sizeof(double), cudaMemcpyHostToDevice, st);
+    *dev = tmp.as<double>();
+    return e;
+}
+
+std::vector<int> orbital_groups(int n_orb) {
+    const int ng = (n_orb + kMaxOT - 1) / kMaxOT;
+    std::vector<int> g(ng, n_orb / ng);
+    for (int i = 0; i < n_orb % ng; ++i) ++g[i];
+    return g;
+}
+
+bool g_direct_profiling = false;
+std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_direct_pairs;
+
+}  // namespace
+
+struct bltc_plan_s {
+    HostPlan hp;
+    bool on_device = false;
+    int device = 0;
+    double upload_ms = 0;
+    // static device state
+    DevBuf<double4> src_rec, tgt_rec_own;
+    const double4* tgt_rec = nullptr;
+    DevBuf<int32_t> src_perm, tgt_perm_own;
+    const int32_t* tgt_perm = nullptr;
+    DevBuf<int32_t> b_begin, b_count, b_nseg, slot_begin, slot_end, far_slots;
+    DevBuf<int64_t> b_partial_base;
+    DevBuf<double> slot_nodes, what;
+    DevBuf<Range> near_ranges;
+    DevBuf<WorkItem> far_items[2], near_items[2];
+    // per-convolve scratch (sized for kMaxOT)
+    DevBuf<double> fsrc, ftgt_own, fhat, partial, f_stage, out_stage;
+    int last_ot = 0;
+    // profiling
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;     // (BLTC_NUM_PHASES + 1) per orbital group
+    int events_used = 0;
+    ~bltc_plan_s() { for (cudaEvent_t e : events) cudaEventDestroy(e); }
+};
+
+namespace {
+
+int check_create_args(bltc_handle* h, const double* sources, int64_t N, double theta, int degree,
+                      int batch_size, int leaf_size) {
+    if (!h) return fail(BLTC_EINVAL, "handle pointer is NULL");
+    if (!sources) return fail(BLTC_EINVAL, "sources is NULL");
+    if (N <= 0 || N > 2000000000LL) return fail(BLTC_EINVAL, "N must be in [1, 2e9]");
+    if (!(theta >= 0.0) || !(theta < 1.0)) return fail(BLTC_EINVAL, "theta must satisfy 0 <= theta < 1");
+    if (degree < 1 || degree > 20) return fail(BLTC_EINVAL, "interp_degree must be in [1, 20]");
+    if (batch_size < 1 || leaf_size < 1) return fail(BLTC_EINVAL, "batch_size and leaf_size must be >= 1");
+    return BLTC_OK;
+}
+
+int build_plan_guarded(bltc_plan_s* pl, const double* targets, const double* sources, int64_t N,
+                       double theta, int degree, int batch_size, int leaf_size, int sms) {
+    try {
+        build_host_plan(pl->hp, targets, sources, N, theta, degree, batch_size, leaf_size, sms);
+    } catch (const std::bad_alloc&) {
+        return fail(BLTC_ENOMEM, "host allocation failed while building the plan");
+    } catch (const std::exception& e) {
+        return fail(BLTC_EINVAL, e.what());
+    }
+    return BLTC_OK;
+}
+
+std::vector<int32_t> to_i32(const std::vector<int64_t>& v) {
+    std::vector<int32_t> o(v.size());
+    for (size_t i = 0; i < v.size(); ++i) o[i] = (int32_t)v[i];
+    return o;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bltc_last_error(void) { return g_err.c_str(); }
+const char* bltc_version(void) { return "bltc-b200 0.1 (sm_100a)"; }
+
+int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* sources,
+                          const double* weights, int64_t N, double theta, int interp_degree,
+                          int batch_size, int leaf_size) {
+    (void)weights;
+    int rc = check_create_args(h, sources, N, theta, interp_degree, batch_size, leaf_size);
+    if (rc) return rc;
+    bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
+    if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
+    rc = build_plan_guarded(pl, targets, sources, N, theta, interp_degree, batch_size, leaf_size, 148);
+    if (rc) { delete pl; return rc; }
+    *h = pl;
+    return BLTC_OK;
+}
+
+int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                int64_t N, double theta, int interp_degree, int batch_size, int leaf_size) {
+    int rc = check_create_args(h, sources, N, theta, interp_degree, batch_size, leaf_size);
+    if (rc) return rc;
+    if (!weights) return fail(BLTC_EINVAL, "weights is NULL");
+    int dev = 0, sms = 0;
+    BLTC_CUDA(cudaGetDevice(&dev));
+    BLTC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    // host copies of the coordinates (the tree is built on the host, timed separately)
+    const bool same = (targets == nullptr || targets == sources);
+    std::vector<double> hs, ht, hw;
+    try {
+        hs.resize(3 * (size_t)N); hw.resize((size_t)N);
+        if (!same) ht.resize(3 * (size_t)N);
+    } catch (const std::bad_alloc&) { return fail(BLTC_ENOMEM, "host allocation failed"); }
+    BLTC_CUDA(cudaMemcpy(hs.data(), sources, hs.size() * sizeof(double), cudaMemcpyDefault));
+    BLTC_CUDA(cudaMemcpy(hw.data(), weights, hw.size() * sizeof(double), cudaMemcpyDefault));
+    if (!same) BLTC_CUDA(cudaMemcpy(ht.data(), targets, ht.size() * sizeof(double), cudaMemcpyDefault));
+
+    bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
+    if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
+    rc = build_plan_guarded(pl, same ? nullptr : ht.data(), hs.data(), N, theta, interp_degree,
+                            batch_size, leaf_size, sms);
+    if (rc) { delete pl; return rc; }
+    pl->device = dev;
+
+    const auto t0 = std::chrono::steady_clock::now();
+    HostPlan& hp = pl->hp;
+#define BLTC_TRY_OR_FREE(call)                                                                 \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess) {                                                              \
+            cudaGetLastError(); delete pl;                                                     \
+            return fail(e__ == cudaErrorMemoryAllocation ? BLTC_ENOMEM : BLTC_ECUDA,           \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                  \
+        }                                                                                      \
+    } while (0)
+    // tree-ordered records
+    {
+        DevBuf<double> d_coords, d_w;
+        BLTC_TRY_OR_FREE(d_coords.upload(hs));
+        BLTC_TRY_OR_FREE(d_w.upload(hw));
+        BLTC_TRY_OR_FREE(pl->src_perm.upload(to_i32(hp.src.perm)));
+        BLTC_TRY_OR_FREE(pl->src_rec.ensure((size_t)N));
+        BLTC_TRY_OR_FREE(launch_pack_records(d_coords.p, d_w.p, pl->src_perm.p, N, pl->src_rec.p, nullptr));
+        if (hp.shared_order) {
+            pl->tgt_rec = pl->src_rec.p; pl->tgt_perm = pl->src_perm.p;
+        } else {
+            if (!same) BLTC_TRY_OR_FREE(d_coords.upload(ht));
+            BLTC_TRY_OR_FREE(pl->tgt_perm_own.upload(to_i32(hp.tgt.perm)));
+            BLTC_TRY_OR_FREE(pl->tgt_rec_own.ensure((size_t)N));
+            BLTC_TRY_OR_FREE(launch_pack_records(d_coords.p, nullptr, pl->tgt_perm_own.p, N, pl->tgt_rec_own.p, nullptr));
+            pl->tgt_rec = pl->tgt_rec_own.p; pl->tgt_perm = pl->tgt_perm_own.p;
+        }
+        BLTC_TRY_OR_FREE(cudaDeviceSynchronize());
+    }
+    // batches, lists, work items
+    {
+        const size_t nb = hp.b_begin.size();
+        std::vector<int32_t> bb(nb), bc(nb), bs(nb);
+        for (size_t b = 0; b < nb; ++b) {
+            bb[b] = (int32_t)hp.b_begin[b]; bc[b] = (int32_t)(hp.b_end[b] - hp.b_begin[b]);
+            bs[b] = hp.b_nseg_far[b] + hp.b_nseg_near[b];
+        }
+        BLTC_TRY_OR_FREE(pl->b_begin.upload(bb));
+        BLTC_TRY_OR_FREE(pl->b_count.upload(bc));
+        BLTC_TRY_OR_FREE(pl->b_nseg.upload(bs));
+        BLTC_TRY_OR_FREE(pl->b_partial_base.upload(hp.b_partial_base));
+        const size_t ns = hp.cluster_of_slot.size();
+        std::vector<int32_t> sb(ns), se(ns);
+        for (size_t s = 0; s < ns; ++s) {
+            sb[s] = (int32_t)hp.src.cl[hp.cluster_of_slot[s]].begin;
+            se[s] = (int32_t)hp.src.cl[hp.cluster_of_slot[s]].end;
+        }
+        BLTC_TRY_OR_FREE(pl->slot_begin.upload(sb));
+        BLTC_TRY_OR_FREE(pl->slot_end.upload(se));
+        BLTC_TRY_OR_FREE(pl->slot_nodes.upload(hp.slot_nodes));
+        BLTC_TRY_OR_FREE(pl->far_slots.upload(hp.far_slots));
+        BLTC_TRY_OR_FREE(pl->near_ranges.upload(hp.near_ranges));
+        for (int rv = 0; rv < 2; ++rv) {
+            BLTC_TRY_OR_FREE(pl->far_items[rv].upload(hp.far_items[rv]));
+            BLTC_TRY_OR_FREE(pl->near_items[rv].upload(hp.near_items[rv]));
+        }
+        // f-independent proxy weights what_k (Eq. (35) right with q_j = w_j)
+        BLTC_TRY_OR_FREE(pl->what.ensure(ns * (size_t)hp.P));
+        BLTC_TRY_OR_FREE(launch_upward(0, (int)ns, pl->slot_begin.p, pl->slot_end.p, pl->slot_nodes.p,
+                                       hp.degree, pl->src_rec.p, nullptr, pl->what.p, nullptr));
+        BLTC_TRY_OR_FREE(cudaDeviceSynchronize());
+    }
+#undef BLTC_TRY_OR_FREE
+    pl->upload_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    pl->on_device = true;
+    *h = pl;
+    return BLTC_OK;
+}
+
+int bltc_destroy(bltc_handle h) {
+    if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    delete h;
+    return BLTC_OK;
+}
+
+int bltc_get_stats(bltc_handle h, bltc_stats* s) {
+    if (!h || !s) return fail(BLTC_EINVAL, "NULL argument");
+    const HostPlan& hp = h->hp;
+    std::memset(s, 0, sizeof *s);
+    s->n_points = hp.N;
+    s->n_clusters = (int64_t)hp.src.cl.size();
+    s->n_leaves = (int64_t)hp.src.leaves.size();
+    s->n_batches = (int64_t)hp.b_begin.size();
+    s->n_far = (int64_t)hp.far_idx.size();
+    s->n_near = (int64_t)hp.near_idx.size();
+    s->far_evals = hp.far_evals;
+    s->near_evals = hp.near_evals;
+    s->n_proxy_clusters = (int64_t)hp.cluster_of_slot.size();
+    s->upward_pairs = hp.upward_pairs;
+    s->n_far_items = (int64_t)hp.far_items[1].size();
+    s->n_near_items = (int64_t)hp.near_items[1].size();
+    s->partial_len = hp.partial_len;
+    s->shared_batches = hp.shared_order ? 1 : 0;
+    s->interp_degree = hp.degree;
+    s->theta = hp.theta;
+    s->build_ms = hp.build_ms;
+    s->upload_ms = h->upload_ms;
+    return BLTC_OK;
+}
+
+int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
+                     int64_t* cl_begin, int64_t* cl_end, double* cl_lo, double* cl_hi,
+                     int32_t* cl_parent, int32_t* cl_nchild, int64_t* b_begin, int64_t* b_end,
+                     int64_t* far_ptr, int32_t* far_idx, int64_t* near_ptr, int32_t* near_idx) {
+    if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    const HostPlan& hp = h->hp;
+    if (src_perm) std::memcpy(src_perm, hp.src.perm.data(), hp.src.perm.size() * sizeof(int64_t));
+    if (tgt_perm) std::memcpy(tgt_perm, hp.tgt_perm().data(), hp.tgt_perm().size() * sizeof(int64_t));
+    for (size_t c = 0; c < hp.src.cl.size(); ++c) {
+        const Cluster& C = hp.src.cl[c];
+        if (cl_begin) cl_begin[c] = C.begin;
+        if (cl_end) cl_end[c] = C.end;
+        for (int d = 0; d < 3; ++d) {
+            if (cl_lo) cl_lo[3 * c + d] = C.lo[d];
+            if (cl_hi) cl_hi[3 * c + d] = C.hi[d];
+        }
+        if (cl_parent) cl_parent[c] = C.parent;
+        if (cl_nchild) cl_nchild[c] = C.nchild;
+    }
+    if (b_begin) std::memcpy(b_begin, hp.b_begin.data(), hp.b_begin.size() * sizeof(int64_t));
+    if (b_end) std::memcpy(b_end, hp.b_end.data(), hp.b_end.size() * sizeof(int64_t));
+    if (far_ptr) std::memcpy(far_ptr, hp.far_ptr.data(), hp.far_ptr.size() * sizeof(int64_t));
+    if (near_ptr) std::memcpy(near_ptr, hp.near_ptr.data(), hp.near_ptr.size() * sizeof(int64_t));
+    if (far_idx) std::memcpy(far_idx, hp.far_idx.data(), hp.far_idx.size() * sizeof(int32_t));
+    if (near_idx) std::memcpy(near_idx, hp.near_idx.data(), hp.near_idx.size() * sizeof(int32_t));
+    return BLTC_OK;
+}
+
+int bltc_export_proxy(bltc_handle h, int32_t* proxy_cluster, double* nodes, double* what,
+                      double* fhat, int32_t* ot) {
+    if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    if (!h->on_device) return fail(BLTC_ENODEVICE, "plan has no device state");
+    const HostPlan& hp = h->hp;
+    const size_t ns = hp.cluster_of_slot.size();
+    BLTC_CUDA(cudaDeviceSynchronize());
+    if (proxy_cluster) std::memcpy(proxy_cluster, hp.cluster_of_slot.data(), ns * sizeof(int32_t));
+    if (nodes) std::memcpy(nodes, hp.slot_nodes.data(), hp.slot_nodes.size() * sizeof(double));
+    if (what && ns) BLTC_CUDA(cudaMemcpy(what, h->what.p, ns * hp.P * sizeof(double), cudaMemcpyDeviceToHost));
+    if (fhat && ns && h->last_ot > 0)
+        BLTC_CUDA(cudaMemcpy(fhat, h->fhat.p, ns * hp.P * h->last_ot * sizeof(double), cudaMemcpyDeviceToHost));
+    if (ot) *ot = h->last_ot;
+    return BLTC_OK;
+}
+
+int bltc_set_profiling(bltc_handle h, int enable) {
+    if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    h->profiling = enable != 0;
+    return BLTC_OK;
+}
+
+int bltc_get_phase_ms(bltc_handle h, float ms[BLTC_NUM_PHASES]) {
+    if (!h || !ms) return fail(BLTC_EINVAL, "NULL argument");
+    for (int p = 0; p < BLTC_NUM_PHASES; ++p) ms[p] = 0.f;
+    if (h->events_used == 0) return fail(BLTC_EINVAL, "no profiled convolve has run");
+    BLTC_CUDA(cudaEventSynchronize(h->events[h->events_used - 1]));
+    const int per = BLTC_NUM_PHASES + 1;
+    for (int g = 0; g < h->events_used / per; ++g)
+        for (int p = 0; p < BLTC_NUM_PHASES; ++p) {
+            float t = 0.f;
+            BLTC_CUDA(cudaEventElapsedTime(&t, h->events[g * per + p], h->events[g * per + p + 1]));
+            ms[p] += t;
+        }
+    return BLTC_OK;
+}
+
+int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
+                  int subtract_singularity, bltc_stream stream) {
+    if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    if (!h->on_device) return fail(BLTC_ENODEVICE, "plan was built with bltc_create_host_plan (no device state)");
+    if (!k || !f || !out) return fail(BLTC_EINVAL, "k, f and out must not be NULL");
+    if (n_orb < 1) return fail(BLTC_EINVAL, "n_orb must be >= 1");
+    HostPlan& hp = h->hp;
+    const bool sub = subtract_singularity != 0;
+    if (sub && !hp.same_points) return fail(BLTC_EINVAL, "subtract_singularity requires targets == sources");
+    for (int o = 0; o < n_orb; ++o)
+        if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int64_t N = hp.N;
+
+    // host buffers are staged through device memory inside the call
+    const double* d_f = f;
+    double* d_out = out;
+    const bool out_on_host = !is_device_ptr(out);
+    if (!is_device_ptr(f)) {
+        BLTC_CUDA(h->f_stage.ensure((size_t)n_orb * N));
+        BLTC_CUDA(cudaMemcpyAsync(h->f_stage.p, f, (size_t)n_orb * N * sizeof(double), cudaMemcpyHostToDevice, st));
+        d_f = h->f_stage.p;
+    }
+    if (out_on_host) {
+        BLTC_CUDA(h->out_stage.ensure((size_t)n_orb * N));
+        d_out = h->out_stage.p;
+    }
+
+    const size_t ns = hp.cluster_of_slot.size();
+    BLTC_CUDA(h->fsrc.ensure((size_t)N * kMaxOT));
+    if (!hp.shared_order && sub) BLTC_CUDA(h->ftgt_own.ensure((size_t)N * kMaxOT));
+    BLTC_CUDA(h->fhat.ensure(ns * (size_t)hp.P * kMaxOT));
+    BLTC_CUDA(h->partial.ensure((size_t)hp.partial_len * kMaxOT));
+
+    const std::vector<int> groups = orbital_groups(n_orb);
+    const int per = BLTC_NUM_PHASES + 1;
+    if (h->profiling) {
+        while (h->events.size() < groups.size() * per) {
+            cudaEvent_t e; BLTC_CUDA(cudaEventCreate(&e)); h->events.push_back(e);
+        }
+    }
+    h->events_used = 0;
+    int o0 = 0;
+    for (size_t g = 0; g < groups.size(); ++g) {
+        const int ot = groups[g];
+        const int rv = targets_per_thread(ot) - 1;
+        KNeg nk;
+        for (int o = 0; o < kMaxOT; ++o) nk.nk[o] = o < ot ? -k[o0 + o] : -1.0;
+        cudaEvent_t* ev = h->profiling ? &h->events[g * per] : nullptr;
+        if (ev) BLTC_CUDA(cudaEventRecord(ev[0], st));
+        // a1: gather to tree order
+        BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->src_perm.p, N, h->fsrc.p, st));
+        const double* ftgt = h->fsrc.p;
+        if (!hp.shared_order && sub) {
+            BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->tgt_perm, N, h->ftgt_own.p, st));
+            ftgt = h->ftgt_own.p;
+        }
+        if (ev) BLTC_CUDA(cudaEventRecord(ev[1], st));
+        // a2: upward pass
+        BLTC_CUDA(launch_upward(ot, (int)ns, h->slot_begin.p, h->slot_end.p, h->slot_nodes.p, hp.degree,
+                                h->src_rec.p, h->fsrc.p, h->fhat.p, st));
+        if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
+        // a3: far field
+        BLTC_CUDA(launch_far(ot, sub, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
+                             h->slot_nodes.p, h->what.p, h->fhat.p, hp.degree, h->tgt_rec, ftgt, nk,
+                             h->partial.p, hp.partial_len, st));
+        if (ev) BLTC_CUDA(cudaEventRecord(ev[3], st));
+        // a4: near field
+        BLTC_CUDA(launch_near(ot, sub, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
+                              h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
+        if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
+        // a5: epilogue
+        BLTC_CUDA(launch_epilogue(ot, sub, (int)hp.b_begin.size(), h->b_begin.p, h->b_count.p,
+                                  h->b_partial_base.p, h->b_nseg.p, h->partial.p, hp.partial_len, ftgt, nk,
+                                  h->tgt_perm, d_out, N, o0, st));
+        if (ev) { BLTC_CUDA(cudaEventRecord(ev[5], st)); h->events_used += per; }
+        h->last_ot = ot;
+        o0 += ot;
+    }
+    if (out_on_host) {
+        BLTC_CUDA(cudaMemcpyAsync(out, d_out, (size_t)n_orb * N * sizeof(double), cudaMemcpyDeviceToHost, st));
+        BLTC_CUDA(cudaStreamSynchronize(st));
+    }
+    return BLTC_OK;
+}
+
+int bltc_direct_set_profiling(int enable) { g_direct_profiling = enable != 0; return BLTC_OK; }
+
+int bltc_direct_get_kernel_ms(float* ms) {
+    if (!ms) return fail(BLTC_EINVAL, "NULL argument");
+    *ms = 0.f;
+    if (g_direct_pairs.empty()) return fail(BLTC_EINVAL, "no profiled direct_convolve has run");
+    for (auto& pr : g_direct_pairs) {
+        float t = 0.f;
+        BLTC_CUDA(cudaEventSynchronize(pr.second));
+        BLTC_CUDA(cudaEventElapsedTime(&t, pr.first, pr.second));
+        *ms += t;
+    }
+    return BLTC_OK;
+}
+
+int direct_convolve(const double* targets, const double* f_targets, int64_t M,
+                    const double* sources, const double* weights, const double* f_sources, int64_t N,
+                    const double* k, int n_orb, double* out, int subtract_singularity,
+                    bltc_stream stream) {
+    if (!targets || !sources || !weights || !f_sources || !k || !out)
+        return fail(BLTC_EINVAL, "targets, sources, weights, f_sources, k and out must not be NULL");
+    if (M < 0 || N < 0 || M > 2000000000LL || N > 2000000000LL) return fail(BLTC_EINVAL, "M, N must be in [0, 2e9]");
+    if (n_orb < 1) return fail(BLTC_EINVAL, "n_orb must be >= 1");
+    const bool sub = subtract_singularity != 0;
+    if (sub && !f_targets) return fail(BLTC_EINVAL, "subtract_singularity needs f_targets");
+    for (int o = 0; o < n_orb; ++o)
+        if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    if (M == 0) return BLTC_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    BLTC_CUDA(cudaGetDevice(&dev));
+    BLTC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    TempBuf t_tg, t_ft, t_sr, t_w, t_fs, t_out;
+    const double *d_tg, *d_ft, *d_sr, *d_w, *d_fs;
+    BLTC_CUDA(stage_in(targets, 3 * (size_t)M, t_tg, st, &d_tg));
+    BLTC_CUDA(stage_in(sub ? f_targets : nullptr, (size_t)n_orb * M, t_ft, st, &d_ft));
+    BLTC_CUDA(stage_in(sources, 3 * (size_t)N, t_sr, st, &d_sr));
+    BLTC_CUDA(stage_in(weights, (size_t)N, t_w, st, &d_w));
+    BLTC_CUDA(stage_in(f_sources, (size_t)n_orb * N, t_fs, st, &d_fs));
+    const bool out_on_host = !is_device_ptr(out);
+    double* d_out = out;
+    if (out_on_host) { BLTC_CUDA(t_out.alloc((size_t)n_orb * M * sizeof(double), st)); d_out = t_out.as<double>(); }
+
+    // work decomposition: pseudo-batches of 2048 targets, tiles of 8 groups inside them, and
+    // nsplit equal source segments so that >= ~16 CTAs exist per resident CTA slot
+    constexpr int64_t kPB = 2048;
+    std::vector<WorkItem> items[2];
+    std::vector<Range> ranges;
+    std::vector<int32_t> pb_begin, pb_count, pb_nseg;
+    std::vector<int64_t> pb_base;
+    int nsplit = 1;
+    {
+        const int64_t tiles512 = (M + 511) / 512;
+        const int64_t want = (int64_t)sms * 2 * 8;
+        nsplit = (int)std::min<int64_t>(64, std::max<int64_t>(1, (want + tiles512 - 1) / tiles512));
+        nsplit = (int)std::min<int64_t>(nsplit, std::max<int64_t>(1, N / 256));
+        for (int s = 0; s < nsplit; ++s)
+            ranges.push_back(Range{(int32_t)(N * s / nsplit), (int32_t)(N * (s + 1) / nsplit)});
+        for (int64_t b0 = 0; b0 < M; b0 += kPB) {
+            pb_begin.push_back((int32_t)b0);
+            pb_count.push_back((int32_t)std::min<int64_t>(kPB, M - b0));
+            pb_nseg.push_back(nsplit);
+            pb_base.push_back((int64_t)nsplit * b0);
+        }
+        for (int rv = 0; rv < 2; ++rv) {
+            const int unit = 32 << rv;
+            for (int64_t t0 = 0; t0 < M;) {
+                const int64_t pb = t0 / kPB, pb_end = std::min<int64_t>(M, (pb + 1) * kPB);
+                const int64_t groups = (pb_end - t0 + unit - 1) / unit;
+                int g = 8;
+                if (groups < 8) { g = 1; while (2 * g <= groups) g *= 2; }
+                int gs = 0; while ((1 << gs) < g) ++gs;
+                const int64_t cnt = std::min<int64_t>((int64_t)g * unit, pb_end - t0);
+                for (int s = 0; s < nsplit; ++s)
+                    items[rv].push_back(WorkItem{(int32_t)t0, (int32_t)cnt, gs, s, s + 1, 0,
+                                                 pb_base[pb] + (int64_t)s * pb_count[pb] + (t0 - pb * kPB)});
+                t0 += cnt;
+            }
+        }
+    }
+    const int64_t partial_len = (int64_t)nsplit * M;
+    const size_t npb = pb_begin.size();
+    TempBuf t_src_rec, t_tgt_rec, t_fsrc, t_ftgt, t_partial, t_items[2], t_ranges, t_pbb, t_pbc, t_pbn, t_pbs;
+    BLTC_CUDA(t_src_rec.alloc((size_t)N * sizeof(double4), st));
+    BLTC_CUDA(t_tgt_rec.alloc((size_t)M * sizeof(double4), st));
+    BLTC_CUDA(t_fsrc.alloc((size_t)N * kMaxOT * sizeof(double), st));
+    BLTC_CUDA(t_ftgt.alloc((size_t)M * kMaxOT * sizeof(double), st));
+    BLTC_CUDA(t_partial.alloc((size_t)partial_len * kMaxOT * sizeof(double), st));
+    auto put = [&](TempBuf& t, const void* src, size_t bytes) -> cudaError_t {
+        cudaError_t e = t.alloc(bytes, st);
+        if (e != cudaSuccess) return e;
+        return cudaMemcpyAsync(t.p, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    BLTC_CUDA(put(t_ranges, ranges.data(), ranges.size() * sizeof(Range)));
+    BLTC_CUDA(put(t_pbb, pb_begin.data(), npb * sizeof(int32_t)));
+    BLTC_CUDA(put(t_pbc, pb_count.data(), npb * sizeof(int32_t)));
+    BLTC_CUDA(put(t_pbn, pb_nseg.data(), npb * sizeof(int32_t)));
+    BLTC_CUDA(put(t_pbs, pb_base.data(), npb * sizeof(int64_t)));
+    BLTC_CUDA(launch_pack_records(d_sr, d_w, nullptr, N, t_src_rec.as<double4>(), st));
+    BLTC_CUDA(launch_pack_records(d_tg, nullptr, nullptr, M, t_tgt_rec.as<double4>(), st));
+
+    const std::vector<int> groups = orbital_groups(n_orb);
+    if (g_direct_profiling) {
+        for (auto& pr : g_direct_pairs) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+        g_direct_pairs.clear();
+    }
+    int o0 = 0;
+    for (size_t g = 0; g < groups.size(); ++g) {
+        const int ot = groups[g];
+        const int rv = targets_per_thread(ot) - 1;
+        if (!t_items[rv].p)
+            BLTC_CUDA(put(t_items[rv], items[rv].data(), items[rv].size() * sizeof(WorkItem)));
+        KNeg nk;
+        for (int o = 0; o < kMaxOT; ++o) nk.nk[o] = o < ot ? -k[o0 + o] : -1.0;
+        BLTC_CUDA(launch_gather(d_fs, N, o0, ot, nullptr, N, t_fsrc.as<double>(), st));
+        if (sub) BLTC_CUDA(launch_gather(d_ft, M, o0, ot, nullptr, M, t_ftgt.as<double>(), st));
+        cudaEvent_t ea = nullptr, eb = nullptr;
+        if (g_direct_profiling) {
+            BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
+            BLTC_CUDA(cudaEventRecord(ea, st));
+        }
+        BLTC_CUDA(launch_near(ot, sub, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
+                              t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
+                              t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
+        if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }
+        BLTC_CUDA(launch_epilogue(ot, sub, (int)npb, t_pbb.as<int32_t>(), t_pbc.as<int32_t>(),
+                                  t_pbs.as<int64_t>(), t_pbn.as<int32_t>(), t_partial.as<double>(), partial_len,
+                                  t_ftgt.as<double>(), nk, nullptr, d_out, M, o0, st));
+        o0 += ot;
+    }
+    if (out_on_host) {
+        BLTC_CUDA(cudaMemcpyAsync(out, d_out, (size_t)n_orb * M * sizeof(double), cudaMemcpyDeviceToHost, st));
+        BLTC_CUDA(cudaStreamSynchronize(st));
+    }
+    return BLTC_OK;
+}
+
+int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream) {
+    if (!tflops || iters < 1) return fail(BLTC_EINVAL, "bad argument");
+    float ms = 0.f; double dfma = 0.0;
+    BLTC_CUDA(launch_fp64_probe(iters, &ms, &dfma, static_cast<cudaStream_t>(stream)));
+    *tflops = 2.0 * dfma / (ms * 1e-3) / 1e12;
+    return BLTC_OK;
+}
+
+}  // extern "C"

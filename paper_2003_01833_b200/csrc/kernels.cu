@@ -1,0 +1,533 @@
+// kernels.cu -- hand-written FP64 CUDA kernels (sm_100a) of the BLTC Yukawa convolution.
+//
+//   near_kernel  (a4, a6)  Eq. (34) PAPER.md:389 / Eq. (32) PAPER.md:371 with the subtraction of Eq. (20)
+//   far_kernel   (a3)      Eq. (35) left PAPER.md:394 on the tensor Chebyshev grid of Eq. (37)
+//   upward_kernel(a2)      Eq. (35) right with the barycentric form Eq. (38)-(39) PAPER.md:416-421
+//   gather / pack / epilogue (a1, a5)  Eq. (18),(20),(21) PAPER.md:193-208
+//
+// Mapping (all three pair kernels): one CTA = 8 warps = one work item = (tile of targets) x (list
+// segment).  A thread owns R targets in registers (R*32 per warp = one "group"); a tile has
+// 2^gshift <= 8 groups; the 8 warps are laid out as groups x S source-split ways (S = 8 >> gshift),
+// so small batches still fill every warp.  Sources / proxy points are staged in shared memory and
+// read by broadcast (all lanes of a warp read the same source).  The S partial sums are reduced
+// through shared memory in a fixed order and written to a per-(batch, segment) slice of the
+// partial buffer; the epilogue adds the slices in a fixed order => bitwise reproducible results.
+//
+// The bound is the FP64 pipe ("Roofline"): ~27 (near) / ~22 (far) FP64 instructions
+// per kernel evaluation for one orbital; everything else (LDS, MUFU seed, integer exponent work,
+// loop control) issues in the shadow of the half-rate FP64 pipe.
+#include "kernels.cuh"
+
+#include "fp64_math.cuh"
+
+namespace bltc {
+namespace {
+
+constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
+
+// ------------------------------------------------------------------------------------ a1 / pack
+__global__ void gather_kernel(const double* __restrict__ f, int64_t stride, int o0, int ot,
+                              const int32_t* __restrict__ perm, int64_t n, double* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t src = perm ? (int64_t)perm[i] : i;
+    for (int o = 0; o < ot; ++o) dst[i * ot + o] = f[(int64_t)(o0 + o) * stride + src];
+}
+
+__global__ void pack_kernel(const double* __restrict__ coords, const double* __restrict__ w,
+                            const int32_t* __restrict__ perm, int64_t n, double4* __restrict__ rec) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t s = perm ? (int64_t)perm[i] : i;
+    rec[i] = make_double4(coords[s], coords[n + s], coords[2 * n + s], w ? w[s] : 0.0);
+}
+
+// ------------------------------------------------------------------------------------ a2
+// One CTA per proxy cluster.  Phase A: barycentric Lagrange values L_k(x_j), L_k(y_j), L_k(z_j)
+// for a tile of particles (Eq. (38)-(39); exact node hits give the unit vector, reading R7).
+// Phase B: every thread owns a (k1, k2) row and 4 consecutive k3 and accumulates
+//   qhat_k += L_k1 L_k2 L_k3 q_j      (Eq. (35) right)
+constexpr int kUpTile = 64;
+
+template <int OT>
+__global__ void __launch_bounds__(kThreads)
+upward_kernel(const int32_t* __restrict__ slot_begin, const int32_t* __restrict__ slot_end,
+              const double* __restrict__ slot_nodes, int n1, const double4* __restrict__ src_rec,
+              const double* __restrict__ fsrc, double* __restrict__ out) {
+    constexpr int NC = OT == 0 ? 1 : OT;
+    extern __shared__ double sm[];
+    const int LS = n1 + 3;                       // padded row of L values (pad = 0)
+    double* s_nodes = sm;                        // [3][n1]
+    double* s_L = s_nodes + 3 * n1;              // [kUpTile][3][LS]
+    double* s_q = s_L + kUpTile * 3 * LS;        // [kUpTile][NC]
+    const int tid = threadIdx.x;
+    const int slot = blockIdx.x;
+    const int b = slot_begin[slot], e = slot_end[slot];
+    const int n = n1 - 1;
+    const int P = n1 * n1 * n1;
+    for (int i = tid; i < 3 * n1; i += kThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
+    for (int i = tid; i < kUpTile * 3 * LS; i += kThreads) s_L[i] = 0.0;
+    const int gpr = (n1 + 3) >> 2;               // groups of 4 k3 per (k1, k2) row
+    const int units = n1 * n1 * gpr;
+    for (int u0 = 0; u0 < units; u0 += kThreads) {
+        const int u = u0 + tid;
+        const bool active = u < units;
+        const int row = active ? u / gpr : 0;
+        const int k3a = active ? (u % gpr) * 4 : 0;
+        const int k1 = row / n1, k2 = row % n1;
+        double acc[4][NC];
+#pragma unroll
+        for (int p = 0; p < 4; ++p)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[p][c] = 0.0;
+        for (int j0 = b; j0 < e; j0 += kUpTile) {
+            __syncthreads();
+            for (int t = tid; t < kUpTile * 3; t += kThreads) {
+                const int jj = t / 3, d = t % 3;
+                double* L = s_L + (jj * 3 + d) * LS;
+                if (j0 + jj < e) {
+                    const double4 r = src_rec[j0 + jj];
+                    const double v = d == 0 ? r.x : (d == 1 ? r.y : r.z);
+                    const double* s = s_nodes + d * n1;
+                    int hit = -1;
+                    for (int k = 0; k < n1; ++k) if (v == s[k]) hit = k;
+                    if (hit >= 0) {
+                        for (int k = 0; k < n1; ++k) L[k] = (k == hit) ? 1.0 : 0.0;
+                    } else {
+                        double sum = 0.0;
+                        for (int k = 0; k < n1; ++k) {
+                            const double bk = ((k & 1) ? -1.0 : 1.0) * ((k == 0 || k == n) ? 0.5 : 1.0);
+                            const double t2 = bk / (v - s[k]);
+                            L[k] = t2; sum += t2;
+                        }
+                        const double inv = 1.0 / sum;
+                        for (int k = 0; k < n1; ++k) L[k] *= inv;
+                    }
+                } else {
+                    for (int k = 0; k < n1; ++k) L[k] = 0.0;
+                }
+            }
+            for (int t = tid; t < kUpTile; t += kThreads) {
+                if (j0 + t < e) {
+                    const double w = src_rec[j0 + t].w;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c)
+                        s_q[t * NC + c] = OT == 0 ? w : fsrc[(size_t)(j0 + t) * NC + c] * w;
+                } else {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) s_q[t * NC + c] = 0.0;
+                }
+            }
+            __syncthreads();
+            if (active) {
+                const int cnt = min(kUpTile, e - j0);
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double* L = s_L + jj * 3 * LS;
+                    const double a12 = L[k1] * L[LS + k2];
+                    double q[NC];
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) q[c] = s_q[jj * NC + c];
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) {
+                        const double a = a12 * L[2 * LS + k3a + p];
+#pragma unroll
+                        for (int c = 0; c < NC; ++c) acc[p][c] = fma(a, q[c], acc[p][c]);
+                    }
+                }
+            }
+        }
+        if (active) {
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                const int k3 = k3a + p;
+                if (k3 < n1) {
+                    const size_t kk = (size_t)slot * P + (size_t)(k1 * n1 + k2) * n1 + k3;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) out[kk * NC + c] = acc[p][c];
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ shared pieces
+template <int R, int OT>
+struct TargetRegs {
+    double x[R], y[R], z[R];
+    double f[R][OT];
+    double acc[R][OT];
+    bool valid[R];
+    int tl[R];
+};
+
+template <int R, int OT, bool SUB>
+__device__ __forceinline__ void load_targets(TargetRegs<R, OT>& T, const WorkItem& it, int grp, int lane,
+                                             const double4* __restrict__ tgt_rec,
+                                             const double* __restrict__ ftgt) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        T.tl[r] = (grp * R + r) * 32 + lane;
+        T.valid[r] = T.tl[r] < it.tgt_count;
+        const int ti = it.tgt_begin + (T.valid[r] ? T.tl[r] : 0);    // padded lanes shadow target 0
+        const double4 t = tgt_rec[ti];
+        T.x[r] = t.x; T.y[r] = t.y; T.z[r] = t.z;
+#pragma unroll
+        for (int o = 0; o < OT; ++o) {
+            T.f[r][o] = SUB ? ftgt[(size_t)ti * OT + o] : 0.0;
+            T.acc[r][o] = 0.0;
+        }
+    }
+}
+
+// Reduce the S source-split partial sums of each target (fixed order) and store the tile's slice.
+template <int R, int OT>
+__device__ __forceinline__ void reduce_and_store(TargetRegs<R, OT>& T, const WorkItem& it, int warp,
+                                                 int lane, int split, int S, double* s_red,
+                                                 double* __restrict__ partial, int64_t partial_len) {
+    if (S > 1) {
+        __syncthreads();                                   // staging tile no longer needed
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int o = 0; o < OT; ++o) s_red[((r * OT + o) * 8 + warp) * 32 + lane] = T.acc[r][o];
+        __syncthreads();
+        if (split == 0) {
+            const int G = 8 / S;
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int o = 0; o < OT; ++o) {
+                    double s = T.acc[r][o];
+                    for (int q = 1; q < S; ++q) s += s_red[((r * OT + o) * 8 + warp + q * G) * 32 + lane];
+                    T.acc[r][o] = s;
+                }
+        }
+    }
+    if (split == 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (T.valid[r])
+#pragma unroll
+                for (int o = 0; o < OT; ++o)
+                    partial[(int64_t)o * partial_len + it.partial_off + T.tl[r]] = T.acc[r][o];
+    }
+}
+
+// ------------------------------------------------------------------------------------ a4 / a6
+template <int R, int OT, bool SUB>
+__global__ void __launch_bounds__(kThreads, 2)
+near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
+            const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
+            const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KNeg nk,
+            double* __restrict__ partial, int64_t partial_len) {
+    __shared__ double4 s_rec[kSrcTile];
+    __shared__ double s_f[kSrcTile * OT];
+    __shared__ double s_t16[16];
+    static_assert(sizeof(double4) * kSrcTile >= sizeof(double) * R * OT * 8 * 32, "reduction scratch");
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const WorkItem it = items[blockIdx.x];
+    const int G = 1 << it.gshift, S = 8 >> it.gshift;
+    const int grp = warp & (G - 1), split = warp >> it.gshift;
+    exp_table_init(s_t16, tid);
+    TargetRegs<R, OT> T;
+    load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
+
+    int q = it.list_begin;
+    int at = q < it.list_end ? ranges[q].begin : 0;
+    while (q < it.list_end) {
+        __syncthreads();                                   // previous tile consumed (and table ready)
+        int fill = 0;
+        while (fill < kSrcTile && q < it.list_end) {
+            const int end = ranges[q].end;
+            const int n = min(kSrcTile - fill, end - at);
+            for (int i = tid; i < n; i += kThreads) {
+                s_rec[fill + i] = src_rec[at + i];
+#pragma unroll
+                for (int o = 0; o < OT; ++o) s_f[(fill + i) * OT + o] = fsrc[(size_t)(at + i) * OT + o];
+            }
+            fill += n; at += n;
+            if (at == end) { ++q; if (q < it.list_end) at = ranges[q].begin; }
+        }
+        __syncthreads();
+#pragma unroll 2
+        for (int j = split; j < fill; j += S) {
+            const double4 s = s_rec[j];
+            double sf[OT];
+#pragma unroll
+            for (int o = 0; o < OT; ++o) sf[o] = s_f[j * OT + o];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double dx = T.x[r] - s.x, dy = T.y[r] - s.y, dz = T.z[r] - s.z;
+                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                double rinv, rr;
+                rsqrt_sqrt<true>(r2, rinv, rr);            // r2 == 0: rinv = 0, the term vanishes
+                const double gw = rinv * s.w;
+#pragma unroll
+                for (int o = 0; o < OT; ++o) {
+                    const double ex = exp_neg(nk.nk[o] * rr, s_t16);
+                    const double g = ex * gw;
+                    const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
+                    T.acc[r][o] = fma(g, df, T.acc[r][o]);
+                }
+            }
+        }
+    }
+    reduce_and_store<R, OT>(T, it, warp, lane, split, S, reinterpret_cast<double*>(s_rec), partial, partial_len);
+}
+
+// ------------------------------------------------------------------------------------ a3
+template <int R, int OT, bool SUB>
+__global__ void __launch_bounds__(kThreads, 2)
+far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
+           const double* __restrict__ slot_nodes, const double* __restrict__ what,
+           const double* __restrict__ fhat, int n1, const double4* __restrict__ tgt_rec,
+           const double* __restrict__ ftgt, const KNeg nk, double* __restrict__ partial,
+           int64_t partial_len) {
+    __shared__ double s_w[kProxyTile];
+    __shared__ double s_fh[kProxyTile * OT];
+    __shared__ double s_nodes[3 * 21];
+    __shared__ double s_t16[16];
+    static_assert(kProxyTile >= R * 8 * 32, "reduction scratch fits in s_fh");
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const WorkItem it = items[blockIdx.x];
+    const int G = 1 << it.gshift, S = 8 >> it.gshift;
+    const int grp = warp & (G - 1), split = warp >> it.gshift;
+    exp_table_init(s_t16, tid);
+    TargetRegs<R, OT> T;
+    load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
+
+    const int plane = n1 * n1;
+    const int P = plane * n1;
+    const int planes_per_chunk = max(1, kProxyTile / plane);
+    for (int q = it.list_begin; q < it.list_end; ++q) {
+        const int slot = far_slots[q];
+        for (int k1a = 0; k1a < n1; k1a += planes_per_chunk) {
+            const int k1b = min(n1, k1a + planes_per_chunk);
+            const int npts = (k1b - k1a) * plane;
+            __syncthreads();
+            if (k1a == 0)
+                for (int i = tid; i < 3 * n1; i += kThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
+            const size_t base = (size_t)slot * P + (size_t)k1a * plane;
+            for (int i = tid; i < npts; i += kThreads) {
+                if (SUB) s_w[i] = what[base + i];
+#pragma unroll
+                for (int o = 0; o < OT; ++o) s_fh[i * OT + o] = fhat[(base + i) * OT + o];
+            }
+            __syncthreads();
+            const int rows = (k1b - k1a) * n1;
+            for (int row = split; row < rows; row += S) {
+                const int k1 = k1a + row / n1, k2 = row % n1;
+                double dxy2[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const double dx = T.x[r] - s_nodes[k1], dy = T.y[r] - s_nodes[n1 + k2];
+                    dxy2[r] = fma(dy, dy, dx * dx);
+                }
+                const int pbase = row * n1;
+#pragma unroll 2
+                for (int k3 = 0; k3 < n1; ++k3) {
+                    const double sz = s_nodes[2 * n1 + k3];
+                    const double wv = SUB ? s_w[pbase + k3] : 0.0;
+                    double fv[OT];
+#pragma unroll
+                    for (int o = 0; o < OT; ++o) fv[o] = s_fh[(pbase + k3) * OT + o];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double dz = T.z[r] - sz;
+                        const double r2 = fma(dz, dz, dxy2[r]);
+                        double rinv, rr;
+                        rsqrt_sqrt<false>(r2, rinv, rr);   // MAC keeps targets off the grid (theta < 1)
+#pragma unroll
+                        for (int o = 0; o < OT; ++o) {
+                            const double ex = exp_neg(nk.nk[o] * rr, s_t16);
+                            const double g = ex * rinv;
+                            // fhat_k - f_i what_k: interpolated charges of (f_j - f_i) w_j (reading R11)
+                            const double qk = SUB ? fma(-T.f[r][o], wv, fv[o]) : fv[o];
+                            T.acc[r][o] = fma(g, qk, T.acc[r][o]);
+                        }
+                    }
+                }
+            }
+        }
+    }
+    reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_fh, partial, partial_len);
+}
+
+// ------------------------------------------------------------------------------------ a5
+template <int OT, bool SUB>
+__global__ void __launch_bounds__(kThreads)
+epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__ b_count,
+                const int64_t* __restrict__ b_partial_base, const int32_t* __restrict__ b_nseg,
+                const double* __restrict__ partial, int64_t partial_len, const double* __restrict__ ftgt,
+                const KNeg nk, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
+                int o0) {
+    const int b = blockIdx.x;
+    const int begin = b_begin[b], count = b_count[b], nseg = b_nseg[b];
+    const int64_t base = b_partial_base[b];
+    for (int l = threadIdx.x; l < count; l += kThreads) {
+        const int i = begin + l;
+        const int64_t dst = perm ? (int64_t)perm[i] : (int64_t)i;
+#pragma unroll
+        for (int o = 0; o < OT; ++o) {
+            double s = 0.0;
+            for (int g = 0; g < nseg; ++g) s += partial[(int64_t)o * partial_len + base + (int64_t)g * count + l];
+            double v = -kInv2Pi * s;                               // -2 * S / (4 pi)
+            if (SUB) v = fma(-2.0 / (nk.nk[o] * nk.nk[o]), ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2
+            out[(int64_t)(o0 + o) * stride + dst] = v;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ probe
+__global__ void __launch_bounds__(kThreads)
+fp64_probe_kernel(int iters, double seed, double* sink) {
+    double a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = seed + (double)(threadIdx.x + i);
+    const double m = 1.0 + 1e-9 * seed, c = 1e-12;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 64; ++u)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    if (s == 123.456) sink[0] = s;
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t bytes) {
+    if (bytes > 48 * 1024) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// ===================================================================================== launchers
+cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
+                          int64_t n, double* dst, cudaStream_t st) {
+    if (n == 0) return cudaSuccess;
+    gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(f, stride, o0, ot, perm, n, dst);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_records(const double* coords, const double* w, const int32_t* perm, int64_t n,
+                                double4* rec, cudaStream_t st) {
+    if (n == 0) return cudaSuccess;
+    pack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(coords, w, perm, n, rec);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const int32_t* slot_end,
+                          const double* slot_nodes, int degree, const double4* src_rec,
+                          const double* fsrc, double* out, cudaStream_t st) {
+    if (nslot == 0) return cudaSuccess;
+    const int n1 = degree + 1;
+    const int nc = ot == 0 ? 1 : ot;
+    const size_t smem = sizeof(double) * (3 * n1 + (size_t)kUpTile * 3 * (n1 + 3) + (size_t)kUpTile * nc);
+    cudaError_t e = cudaSuccess;
+#define BLTC_UP(OTV)                                                                                   \
+    case OTV:                                                                                          \
+        e = set_smem(upward_kernel<OTV>, smem);                                                        \
+        if (e != cudaSuccess) return e;                                                                \
+        upward_kernel<OTV><<<nslot, kThreads, smem, st>>>(slot_begin, slot_end, slot_nodes, n1,        \
+                                                          src_rec, fsrc, out);                         \
+        break;
+    switch (ot) {
+        BLTC_UP(0) BLTC_UP(1) BLTC_UP(2) BLTC_UP(3) BLTC_UP(4)
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_UP
+    return cudaGetLastError();
+}
+
+cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
+                       const double* slot_nodes, const double* what, const double* fhat, int degree,
+                       const double4* tgt_rec, const double* ftgt, const KNeg& nk, double* partial,
+                       int64_t partial_len, cudaStream_t st) {
+    if (nitems == 0) return cudaSuccess;
+    const int n1 = degree + 1;
+#define BLTC_FAR(RV, OTV)                                                                               \
+    if (subtract) far_kernel<RV, OTV, true><<<nitems, kThreads, 0, st>>>(items, far_slots, slot_nodes,  \
+        what, fhat, n1, tgt_rec, ftgt, nk, partial, partial_len);                                       \
+    else far_kernel<RV, OTV, false><<<nitems, kThreads, 0, st>>>(items, far_slots, slot_nodes, what,    \
+        fhat, n1, tgt_rec, ftgt, nk, partial, partial_len);
+    switch (ot) {
+        case 1: BLTC_FAR(2, 1) break;
+        case 2: BLTC_FAR(2, 2) break;
+        case 3: BLTC_FAR(1, 3) break;
+        case 4: BLTC_FAR(1, 4) break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_FAR
+    return cudaGetLastError();
+}
+
+cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
+                        const double4* src_rec, const double* fsrc, const double4* tgt_rec,
+                        const double* ftgt, const KNeg& nk, double* partial, int64_t partial_len,
+                        cudaStream_t st) {
+    if (nitems == 0) return cudaSuccess;
+#define BLTC_NEAR(RV, OTV)                                                                              \
+    if (subtract) near_kernel<RV, OTV, true><<<nitems, kThreads, 0, st>>>(items, ranges, src_rec, fsrc, \
+        tgt_rec, ftgt, nk, partial, partial_len);                                                       \
+    else near_kernel<RV, OTV, false><<<nitems, kThreads, 0, st>>>(items, ranges, src_rec, fsrc,         \
+        tgt_rec, ftgt, nk, partial, partial_len);
+    switch (ot) {
+        case 1: BLTC_NEAR(2, 1) break;
+        case 2: BLTC_NEAR(2, 2) break;
+        case 3: BLTC_NEAR(1, 3) break;
+        case 4: BLTC_NEAR(1, 4) break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_NEAR
+    return cudaGetLastError();
+}
+
+cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
+                            const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
+                            int64_t partial_len, const double* ftgt, const KNeg& nk, const int32_t* perm,
+                            double* out, int64_t stride, int o0, cudaStream_t st) {
+    if (nbatch == 0) return cudaSuccess;
+#define BLTC_EPI(OTV)                                                                                  \
+    case OTV:                                                                                          \
+        if (subtract) epilogue_kernel<OTV, true><<<nbatch, kThreads, 0, st>>>(b_begin, b_count,        \
+            b_partial_base, b_nseg, partial, partial_len, ftgt, nk, perm, out, stride, o0);            \
+        else epilogue_kernel<OTV, false><<<nbatch, kThreads, 0, st>>>(b_begin, b_count,                \
+            b_partial_base, b_nseg, partial, partial_len, ftgt, nk, perm, out, stride, o0);            \
+        break;
+    switch (ot) {
+        BLTC_EPI(1) BLTC_EPI(2) BLTC_EPI(3) BLTC_EPI(4)
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_EPI
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStream_t st) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    double* sink = nullptr;
+    e = cudaMalloc(&sink, sizeof(double));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int grid = sms * 8;
+    fp64_probe_kernel<<<grid, kThreads, 0, st>>>(4, 1.0, sink);          // warm-up
+    cudaEventRecord(a, st);
+    fp64_probe_kernel<<<grid, kThreads, 0, st>>>(iters, 1.0, sink);
+    cudaEventRecord(b, st);
+    e = cudaEventSynchronize(b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, a, b);
+    *dfma_count = (double)grid * kThreads * (double)iters * 64.0 * 8.0;
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(sink);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+}  // namespace bltc

@@ -1,0 +1,54 @@
+// kernels.cuh -- launchers of the sm_100a kernels of the BLTC hot path.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "plan_host.hpp"
+
+namespace bltc {
+
+constexpr int kMaxOT = 4;          // orbitals processed together in one pass (register tile)
+constexpr int kThreads = 256;      // 8 warps per CTA
+constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (near field / direct)
+constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field)
+
+// targets per thread for an orbital tile of width ot
+inline int targets_per_thread(int ot) { return ot <= 2 ? 2 : 1; }
+
+struct KNeg { double nk[kMaxOT]; };    // -k_o of the orbital tile (kernel parameter -> constant bank)
+
+// a1: f[o0+o][perm[i]] -> dst[i][ot] (tree order, orbital-interleaved)
+cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
+                          int64_t n, double* dst, cudaStream_t st);
+
+// pack SoA coordinates (+ weights) into double4 records; perm == nullptr: identity
+cudaError_t launch_pack_records(const double* coords, const double* w, const int32_t* perm, int64_t n,
+                                double4* rec, cudaStream_t st);
+
+// a2: proxy charges.  ot == 0: what[slot][P] from w;  ot >= 1: fhat[slot][P][ot] from f*w
+cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const int32_t* slot_end,
+                          const double* slot_nodes, int degree, const double4* src_rec,
+                          const double* fsrc, double* out, cudaStream_t st);
+
+// a3: far field
+cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
+                       const double* slot_nodes, const double* what, const double* fhat, int degree,
+                       const double4* tgt_rec, const double* ftgt, const KNeg& nk, double* partial,
+                       int64_t partial_len, cudaStream_t st);
+
+// a4 / a6: near field and brute-force direct sum (same kernel, different work items)
+cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
+                        const double4* src_rec, const double* fsrc, const double4* tgt_rec,
+                        const double* ftgt, const KNeg& nk, double* partial, int64_t partial_len,
+                        cudaStream_t st);
+
+// a5: out[o0+o][perm[i]] = -2 ( (far + near)/(4 pi) + [subtract] f_i / k_o^2 )
+cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
+                            const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
+                            int64_t partial_len, const double* ftgt, const KNeg& nk, const int32_t* perm,
+                            double* out, int64_t stride, int o0, cudaStream_t st);
+
+// roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed
+cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStream_t st);
+
+}  // namespace bltc

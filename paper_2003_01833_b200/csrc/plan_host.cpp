@@ -1,0 +1,337 @@
+// plan_host.cpp -- see plan_host.hpp.  Compiled with -ffp-contract=off: every MAC and
+// midpoint expression below is evaluated in plain IEEE double, in the written order, so that
+// the decisions are reproducible (readings R4-R8).
+#include "plan_host.hpp"
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <numeric>
+#include <stdexcept>
+
+namespace bltc {
+namespace {
+
+constexpr double kSqrt2 = 1.4142135623730951;
+constexpr double kPi = 3.14159265358979323846;
+
+struct TreeBuilder {
+    const double* c[3];
+    int64_t max_leaf;
+    Tree& t;
+    std::vector<int64_t> tmp;
+    std::vector<uint8_t> code;
+
+    TreeBuilder(Tree& tree, const double* x, const double* y, const double* z, int64_t n, int64_t ml)
+        : c{x, y, z}, max_leaf(ml), t(tree), tmp(n), code(n) {
+        t.perm.resize(n);
+        std::iota(t.perm.begin(), t.perm.end(), int64_t(0));
+    }
+
+    // bisection at the box midpoint, children shrunk to their particles.
+    int subdivide(int64_t b, int64_t e, int parent, int level) {
+        const int id = (int)t.cl.size();
+        t.cl.emplace_back();
+        {
+            Cluster& C = t.cl.back();
+            C.begin = b; C.end = e; C.parent = parent; C.level = level;
+            for (int d = 0; d < 3; ++d) {
+                double lo = c[d][t.perm[b]], hi = lo;
+                for (int64_t i = b + 1; i < e; ++i) {
+                    const double v = c[d][t.perm[i]];
+                    lo = v < lo ? v : lo;
+                    hi = v > hi ? v : hi;
+                }
+                C.lo[d] = lo; C.hi[d] = hi;
+            }
+        }
+        if (e - b <= max_leaf) return id;                         // R4: leaf iff count <= N_L
+        double ext[3], longest = 0.0, mid[3];
+        bool cut[3];
+        int ncut = 0;
+        for (int d = 0; d < 3; ++d) {
+            ext[d] = t.cl[id].hi[d] - t.cl[id].lo[d];
+            longest = ext[d] > longest ? ext[d] : longest;
+        }
+        for (int d = 0; d < 3; ++d) {                             // R5: aspect-ratio rule sqrt(2)
+            cut[d] = ext[d] > 0.0 && ext[d] * kSqrt2 >= longest;
+            ncut += cut[d];
+            mid[d] = 0.5 * (t.cl[id].lo[d] + t.cl[id].hi[d]);
+        }
+        if (ncut == 0) return id;                                 // all particles coincide
+        int64_t count[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int64_t i = b; i < e; ++i) {
+            const int64_t p = t.perm[i];
+            uint8_t k = 0;
+            if (cut[0] && c[0][p] > mid[0]) k |= 1;               // bit0 x, bit1 y, bit2 z
+            if (cut[1] && c[1][p] > mid[1]) k |= 2;
+            if (cut[2] && c[2][p] > mid[2]) k |= 4;
+            code[i] = k;
+            ++count[k];
+        }
+        int live = 0;
+        for (int q = 0; q < 8; ++q) live += count[q] != 0;
+        if (live < 2) return id;                                  // midpoint rounded onto a face
+        int64_t first[8], cur[8];
+        int64_t at = b;
+        for (int q = 0; q < 8; ++q) { first[q] = cur[q] = at; at += count[q]; }
+        for (int64_t i = b; i < e; ++i) tmp[cur[code[i]]++] = t.perm[i];   // stable
+        std::copy(tmp.begin() + b, tmp.begin() + e, t.perm.begin() + b);
+        for (int q = 0; q < 8; ++q) {
+            if (!count[q]) continue;                              // empty children dropped
+            const int ch = subdivide(first[q], first[q] + count[q], id, level + 1);
+            Cluster& C = t.cl[id];
+            C.child[C.nchild++] = ch;
+        }
+        return id;
+    }
+};
+
+void gather_leaves(const Tree& t, int id, std::vector<int>& out) {
+    if (t.cl[id].nchild == 0) { out.push_back(id); return; }
+    for (int q = 0; q < t.cl[id].nchild; ++q) gather_leaves(t, t.cl[id].child[q], out);
+}
+
+void build_tree(Tree& t, const double* x, const double* y, const double* z, int64_t n, int64_t max_leaf) {
+    t.cl.clear();
+    TreeBuilder tb(t, x, y, z, n, max_leaf);
+    tb.subdivide(0, n, -1, 0);
+    t.leaves.clear();
+    gather_leaves(t, 0, t.leaves);
+}
+
+inline double half_diagonal(const double* lo, const double* hi) {
+    const double ex = hi[0] - lo[0], ey = hi[1] - lo[1], ez = hi[2] - lo[2];
+    return 0.5 * std::sqrt((ex * ex + ey * ey) + ez * ez);
+}
+
+// Algorithm 3 ComputePotential, decision part only (text PAPER.md:434).
+struct Traversal {
+    const HostPlan& p;
+    const double* blo; const double* bhi;
+    double rB;
+    std::vector<int32_t>& far; std::vector<int32_t>& near;
+
+    void visit(int c) {
+        const Cluster& C = p.src.cl[c];
+        const double rC = half_diagonal(C.lo, C.hi);
+        const double dx = 0.5 * (blo[0] + bhi[0]) - 0.5 * (C.lo[0] + C.hi[0]);
+        const double dy = 0.5 * (blo[1] + bhi[1]) - 0.5 * (C.lo[1] + C.hi[1]);
+        const double dz = 0.5 * (blo[2] + bhi[2]) - 0.5 * (C.lo[2] + C.hi[2]);
+        const double R = std::sqrt((dx * dx + dy * dy) + dz * dz);
+        const bool separated = (rB + rC) < p.theta * R;           // Eq. (36) left, R6
+        bool big = (int64_t)p.P < (C.end - C.begin);              // Eq. (36) right
+        if (C.hi[0] == C.lo[0] || C.hi[1] == C.lo[1] || C.hi[2] == C.lo[2]) big = false;   // R8
+        if (separated && big) { far.push_back(c); return; }
+        if (!separated) {
+            if (C.nchild == 0) { near.push_back(c); return; }
+            for (int q = 0; q < C.nchild; ++q) visit(C.child[q]);
+            return;
+        }
+        near.push_back(c);                                        // R10: whole cluster, no descent
+    }
+};
+
+int ilog2_floor(int v) { int s = 0; while ((2 << s) <= v) ++s; return s; }
+
+// Tiles of a batch: binary decomposition of its target groups into tiles of 8/4/2/1 groups,
+// so every warp of an 8-warp CTA has work (S = 8 / groups source-split ways).
+void make_tiles(int64_t tb, int64_t te, int unit, std::vector<std::pair<int32_t, int32_t>>& tiles,
+                std::vector<int>& gshift) {
+    tiles.clear(); gshift.clear();
+    int64_t pos = tb;
+    int groups = (int)((te - tb + unit - 1) / unit);
+    while (groups > 0) {
+        const int g = std::min(8, 1 << ilog2_floor(groups));
+        const int64_t cnt = std::min<int64_t>((int64_t)g * unit, te - pos);
+        tiles.emplace_back((int32_t)pos, (int32_t)cnt);
+        gshift.push_back(ilog2_floor(g));
+        pos += cnt; groups -= g;
+    }
+}
+
+}  // namespace
+
+void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
+                     double theta, int degree, int batch_size, int leaf_size, int sm_count) {
+    const auto t0 = std::chrono::steady_clock::now();
+    if (!sources) throw std::invalid_argument("sources is NULL");
+    if (N <= 0 || N > (int64_t)2000000000) throw std::invalid_argument("N must be in [1, 2e9]");
+    if (!(theta >= 0.0) || !(theta < 1.0)) throw std::invalid_argument("theta must be in [0, 1)");
+    if (degree < 1 || degree > 20) throw std::invalid_argument("interp_degree must be in [1, 20]");
+    if (batch_size < 1 || leaf_size < 1) throw std::invalid_argument("batch_size and leaf_size must be >= 1");
+    p = HostPlan();
+    p.N = N; p.M = N; p.theta = theta; p.degree = degree;
+    p.P = (degree + 1) * (degree + 1) * (degree + 1);
+    p.leaf_size = leaf_size; p.batch_size = batch_size;
+    p.same_points = (targets == nullptr || targets == sources);
+    p.shared_order = p.same_points && batch_size == leaf_size;
+    const double* sx = sources; const double* sy = sources + N; const double* sz = sources + 2 * N;
+
+    // Algorithm 3 line 1: tree of source clusters and set of target batches
+    build_tree(p.src, sx, sy, sz, N, leaf_size);
+    const Tree* bt = &p.src;
+    if (!p.shared_order) {
+        const double* t = p.same_points ? sources : targets;
+        build_tree(p.tgt, t, t + N, t + 2 * N, N, batch_size);
+        bt = &p.tgt;
+    }
+    const int nb = (int)bt->leaves.size();
+    p.b_begin.resize(nb); p.b_end.resize(nb); p.b_lo.resize(3 * (size_t)nb); p.b_hi.resize(3 * (size_t)nb);
+    for (int b = 0; b < nb; ++b) {
+        const Cluster& L = bt->cl[bt->leaves[b]];
+        p.b_begin[b] = L.begin; p.b_end[b] = L.end;
+        for (int d = 0; d < 3; ++d) { p.b_lo[3 * b + d] = L.lo[d]; p.b_hi[3 * b + d] = L.hi[d]; }
+    }
+
+    // line 3, decisions: per-batch interaction lists ("precomputed for each target batch")
+    p.far_ptr.assign(nb + 1, 0); p.near_ptr.assign(nb + 1, 0);
+    for (int b = 0; b < nb; ++b) {
+        p.far_ptr[b] = (int64_t)p.far_idx.size(); p.near_ptr[b] = (int64_t)p.near_idx.size();
+        Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
+                     p.far_idx, p.near_idx};
+        tr.visit(0);
+        const int64_t nt = p.b_end[b] - p.b_begin[b];
+        p.far_evals += nt * p.P * ((int64_t)p.far_idx.size() - p.far_ptr[b]);
+        for (size_t q = (size_t)p.near_ptr[b]; q < p.near_idx.size(); ++q)
+            p.near_evals += nt * (p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin);
+    }
+    p.far_ptr[nb] = (int64_t)p.far_idx.size(); p.near_ptr[nb] = (int64_t)p.near_idx.size();
+
+    // proxy slots: clusters that appear in some far list (R9), with their Chebyshev grids Eq. (37)
+    const int ncl = (int)p.src.cl.size();
+    const int n1 = degree + 1;
+    p.slot_of_cluster.assign(ncl, -1);
+    for (int32_t c : p.far_idx) p.slot_of_cluster[c] = 0;
+    for (int c = 0; c < ncl; ++c)
+        if (p.slot_of_cluster[c] == 0) {
+            p.slot_of_cluster[c] = (int32_t)p.cluster_of_slot.size();
+            p.cluster_of_slot.push_back(c);
+            p.upward_pairs += p.src.cl[c].end - p.src.cl[c].begin;
+        }
+    p.slot_nodes.resize(p.cluster_of_slot.size() * 3 * (size_t)n1);
+    for (size_t s = 0; s < p.cluster_of_slot.size(); ++s) {
+        const Cluster& C = p.src.cl[p.cluster_of_slot[s]];
+        for (int d = 0; d < 3; ++d) {
+            const double mid = 0.5 * (C.lo[d] + C.hi[d]);
+            const double half = 0.5 * (C.hi[d] - C.lo[d]);
+            for (int k = 0; k < n1; ++k)
+                p.slot_nodes[(s * 3 + d) * n1 + k] = mid + half * std::cos((kPi * k) / degree);
+        }
+    }
+
+    // ---- B200 work decomposition -------------------------------------------------------
+    // Per batch: near clusters -> merged contiguous source ranges; far clusters -> slot ids.
+    // Lists are cut into segments so that (tiles x segments) gives >= ~32 work items per
+    // resident CTA slot (2 CTAs/SM), each CTA slot then sees many items sorted by cost.
+    const int cta_slots = std::max(1, sm_count) * 2;
+    std::vector<std::vector<Range>> merged(nb);
+    std::vector<int64_t> near_src(nb, 0);
+    double near_cost = 0, far_cost = 0;            // in (target group of 64) x (source) units
+    for (int b = 0; b < nb; ++b) {
+        std::vector<Range>& r = merged[b];
+        for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
+            const Cluster& C = p.src.cl[p.near_idx[q]];
+            r.push_back(Range{(int32_t)C.begin, (int32_t)C.end});
+        }
+        std::sort(r.begin(), r.end(), [](const Range& a, const Range& c) { return a.begin < c.begin; });
+        size_t o = 0;
+        for (size_t i = 0; i < r.size(); ++i) {
+            if (o > 0 && r[o - 1].end == r[i].begin) r[o - 1].end = r[i].end;
+            else r[o++] = r[i];
+        }
+        r.resize(o);
+        for (const Range& g : r) near_src[b] += g.end - g.begin;
+        const double groups = (double)((p.b_end[b] - p.b_begin[b] + 63) / 64);
+        near_cost += groups * (double)near_src[b];
+        far_cost += groups * (double)(p.far_ptr[b + 1] - p.far_ptr[b]) * p.P;
+    }
+    const double near_cap = std::max(512.0, near_cost / (cta_slots * 32.0 * 8.0));
+    const double far_cap = std::max((double)p.P, far_cost / (cta_slots * 32.0 * 8.0));
+
+    p.b_nseg_far.assign(nb, 0); p.b_nseg_near.assign(nb, 0); p.b_partial_base.assign(nb, 0);
+    std::vector<std::pair<int32_t, int32_t>> tiles; std::vector<int> gsh;
+    int64_t partial = 0;
+    for (int b = 0; b < nb; ++b) {
+        const int64_t nt = p.b_end[b] - p.b_begin[b];
+        // near segments: equal source counts, ranges may be cut anywhere
+        std::vector<std::pair<int32_t, int32_t>> nseg_slices;    // [begin, end) into near_ranges
+        if (near_src[b] > 0) {
+            int nseg = (int)std::min<int64_t>(64, (int64_t)std::ceil((double)near_src[b] / near_cap));
+            nseg = std::max(1, nseg);
+            const int64_t per = (near_src[b] + nseg - 1) / nseg;
+            int64_t room = per;
+            int32_t seg_start = (int32_t)p.near_ranges.size();
+            for (const Range& g : merged[b]) {
+                int32_t at = g.begin;
+                while (at < g.end) {
+                    const int32_t take = (int32_t)std::min<int64_t>(room, g.end - at);
+                    p.near_ranges.push_back(Range{at, at + take});
+                    at += take; room -= take;
+                    if (room == 0) {
+                        nseg_slices.emplace_back(seg_start, (int32_t)p.near_ranges.size());
+                        seg_start = (int32_t)p.near_ranges.size(); room = per;
+                    }
+                }
+            }
+            if ((int32_t)p.near_ranges.size() > seg_start)
+                nseg_slices.emplace_back(seg_start, (int32_t)p.near_ranges.size());
+        }
+        // far segments: whole clusters
+        std::vector<std::pair<int32_t, int32_t>> fseg_slices;
+        const int64_t nfar = p.far_ptr[b + 1] - p.far_ptr[b];
+        if (nfar > 0) {
+            const int64_t per = std::max<int64_t>(1, (int64_t)(far_cap / p.P));
+            int64_t nseg = std::min<int64_t>(64, (nfar + per - 1) / per);
+            const int64_t per2 = (nfar + nseg - 1) / nseg;
+            for (int64_t q = 0; q < nfar; q += per2) {
+                const int32_t s0 = (int32_t)p.far_slots.size();
+                for (int64_t u = q; u < std::min(nfar, q + per2); ++u)
+                    p.far_slots.push_back(p.slot_of_cluster[p.far_idx[p.far_ptr[b] + u]]);
+                fseg_slices.emplace_back(s0, (int32_t)p.far_slots.size());
+            }
+        }
+        p.b_nseg_far[b] = (int32_t)fseg_slices.size();
+        p.b_nseg_near[b] = (int32_t)nseg_slices.size();
+        p.b_partial_base[b] = partial;
+        for (int rv = 0; rv < 2; ++rv) {
+            make_tiles(p.b_begin[b], p.b_end[b], 32 << rv, tiles, gsh);
+            for (size_t ti = 0; ti < tiles.size(); ++ti) {
+                const int64_t local = tiles[ti].first - p.b_begin[b];
+                for (size_t s = 0; s < fseg_slices.size(); ++s)
+                    p.far_items[rv].push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                        fseg_slices[s].first, fseg_slices[s].second, 0,
+                        partial + (int64_t)s * nt + local});
+                for (size_t s = 0; s < nseg_slices.size(); ++s)
+                    p.near_items[rv].push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                        nseg_slices[s].first, nseg_slices[s].second, 0,
+                        partial + (int64_t)(fseg_slices.size() + s) * nt + local});
+            }
+        }
+        partial += (int64_t)(fseg_slices.size() + nseg_slices.size()) * nt;
+    }
+    p.partial_len = partial;
+
+    // longest-processing-time-first: the hardware block scheduler hands out CTAs in order
+    auto near_cost_of = [&](const WorkItem& w) {
+        int64_t s = 0;
+        for (int32_t q = w.list_begin; q < w.list_end; ++q) s += p.near_ranges[q].end - p.near_ranges[q].begin;
+        return s << w.gshift;
+    };
+    auto far_cost_of = [&](const WorkItem& w) { return (int64_t)(w.list_end - w.list_begin) << w.gshift; };
+    for (int rv = 0; rv < 2; ++rv) {
+        std::vector<int64_t> key(p.near_items[rv].size());
+        for (size_t i = 0; i < key.size(); ++i) key[i] = near_cost_of(p.near_items[rv][i]);
+        std::vector<size_t> ord(key.size());
+        std::iota(ord.begin(), ord.end(), size_t(0));
+        std::stable_sort(ord.begin(), ord.end(), [&](size_t a, size_t c) { return key[a] > key[c]; });
+        std::vector<WorkItem> sorted(key.size());
+        for (size_t i = 0; i < ord.size(); ++i) sorted[i] = p.near_items[rv][ord[i]];
+        p.near_items[rv].swap(sorted);
+        std::stable_sort(p.far_items[rv].begin(), p.far_items[rv].end(),
+                         [&](const WorkItem& a, const WorkItem& c) { return far_cost_of(a) > far_cost_of(c); });
+    }
+    p.build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+}
+
+}  // namespace bltc

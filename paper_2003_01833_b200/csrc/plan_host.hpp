@@ -1,0 +1,82 @@
+// plan_host.hpp -- host-side plan of the barycentric Lagrange treecode (built once per mesh).
+//
+// Step a0 of the hot path: source-cluster tree, target batches, per-batch
+// MAC interaction lists (Algorithm 3), the per-cluster
+// Chebyshev grids (Eq. (37)), and the B200 work decomposition (tiles, list
+// segments, cost-sorted work items) that the CUDA kernels consume.  Pure C++, no CUDA.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace bltc {
+
+struct Cluster {
+    int64_t begin = 0, end = 0;      // particle range in tree order
+    double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};   // minimal bounding box
+    int parent = -1, level = 0, nchild = 0;
+    int child[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+struct Tree {
+    std::vector<Cluster> cl;         // DFS pre-order, cl[0] = root
+    std::vector<int64_t> perm;       // tree order -> caller index
+    std::vector<int> leaves;         // leaf ids in DFS order
+};
+
+// One CTA's work: a tile of targets (groups of 32*R consecutive targets; 2^gshift groups)
+// against one segment of its batch's far or near list.
+struct WorkItem {
+    int32_t tgt_begin;               // first target (target tree order)
+    int32_t tgt_count;               // targets in the tile
+    int32_t gshift;                  // log2(number of target groups in the tile), 0..3
+    int32_t list_begin, list_end;    // slice of near_ranges / far_slots
+    int32_t pad;
+    int64_t partial_off;             // where this (batch, segment) slice starts in the partial buffer
+};
+
+struct Range { int32_t begin, end; };   // source range in tree order
+
+struct HostPlan {
+    // parameters
+    int64_t N = 0, M = 0;
+    bool same_points = true;         // targets are the sources
+    bool shared_order = true;        // batches are the source leaves (N_B == N_L, same points)
+    double theta = 0;
+    int degree = 0, P = 0, leaf_size = 0, batch_size = 0;
+
+    Tree src, tgt;                   // tgt used only when !shared_order
+    const std::vector<int64_t>& tgt_perm() const { return shared_order ? src.perm : tgt.perm; }
+
+    // batches (target tree order ranges + boxes)
+    std::vector<int64_t> b_begin, b_end;
+    std::vector<double> b_lo, b_hi;  // [nb][3]
+
+    // interaction lists, CSR over batches, cluster ids in traversal order (for export/stats)
+    std::vector<int64_t> far_ptr, near_ptr;
+    std::vector<int32_t> far_idx, near_idx;
+    int64_t far_evals = 0, near_evals = 0;
+
+    // clusters that carry proxy charges ("slots")
+    std::vector<int32_t> slot_of_cluster;      // -1 if never approximated
+    std::vector<int32_t> cluster_of_slot;
+    std::vector<double> slot_nodes;            // [nslot][3][degree+1], Eq. (37)
+    int64_t upward_pairs = 0;                  // sum over slots of cluster size
+
+    // device work decomposition
+    std::vector<Range> near_ranges;            // merged + cut source ranges, per (batch, segment)
+    std::vector<int32_t> far_slots;            // proxy slot ids, per (batch, segment)
+    std::vector<int32_t> b_nseg_far, b_nseg_near;
+    std::vector<int64_t> b_partial_base;       // per batch
+    int64_t partial_len = 0;                   // doubles per orbital
+    std::vector<WorkItem> far_items[2], near_items[2];   // [0]: R = 1 (32 targets/group), [1]: R = 2
+
+    double build_ms = 0;
+};
+
+// Throws std::invalid_argument / std::bad_alloc.  targets == nullptr: targets are the sources.
+// coords: SoA double[3][n].
+void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
+                     double theta, int degree, int batch_size, int leaf_size, int sm_count);
+
+}  // namespace bltc

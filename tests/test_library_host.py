@@ -1,0 +1,89 @@
+"""CPU-only checks of the product library: it loads, exports every symbol include/bltc.h declares,
+validates arguments, and its host plan (tree, batches, MAC lists) is structurally identical to the
+independently written oracle's.  No compute entry point is called (no GPU here)."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2003_01833_b200 import binding as B
+from paper_2003_01833_b200 import inputs as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "bltc.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b((?:bltc_|direct_)\w+)\s*\(", hdr))
+    assert {"bltc_create", "bltc_convolve", "direct_convolve", "bltc_destroy"} <= declared
+    L = B.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == set(B.EXPORTED)
+    assert "sm_100a" in B.bltc_version()
+
+
+def test_argument_validation_without_gpu():
+    c = I.random_cloud(100, seed=0)
+    X = c.coords()
+    for bad in (dict(N=0), dict(theta=1.0), dict(theta=-0.1), dict(interp_degree=0), dict(interp_degree=21),
+                dict(batch_size=0), dict(leaf_size=0)):
+        kw = dict(N=c.N, theta=0.7, interp_degree=4, batch_size=50, leaf_size=50)
+        kw.update(bad)
+        with pytest.raises(B.BltcError) as ei:
+            B.bltc_create_host_plan(None, X, None, **kw)
+        assert ei.value.code == B.BLTC_EINVAL
+    with pytest.raises(ValueError):
+        B.bltc_create_host_plan(None, X.astype(np.float32), None, c.N, 0.7, 4, 50, 50)
+    p = B.bltc_create_host_plan(None, X, None, c.N, 0.7, 4, 50, 50)
+    out = np.empty((1, c.N))
+    with pytest.raises(B.BltcError) as ei:                    # host-only plan cannot compute
+        B.bltc_convolve(p, [1.0], c.f, 1, out, True, stream=0)
+    assert ei.value.code == B.BLTC_ENODEVICE
+    with pytest.raises(B.BltcError):                          # k <= 0
+        B.direct_convolve(X, c.f, c.N, X, c.w, c.f, c.N, [0.0], 1, out, True, stream=0)
+    with pytest.raises(B.BltcError):                          # subtraction needs f at targets
+        B.direct_convolve(X, None, c.N, X, c.w, c.f, c.N, [1.0], 1, out, True, stream=0)
+    B.bltc_destroy(p)
+
+
+CASES = [
+    ("cfg0", lambda: I.config0()),
+    ("cfg0_small_leaves", lambda: I.config0(leaf_size=256, batch_size=256, degree=4)),
+    ("clustered", lambda: I.random_cloud(5000, seed=4, clustered=True, leaf_size=100, batch_size=100, degree=4)),
+    ("second_tree", lambda: I.random_cloud(3000, seed=10, leaf_size=200, batch_size=30, degree=4)),
+    ("ragged", lambda: I.random_cloud(7777, seed=11, leaf_size=333, batch_size=333, degree=3, theta=0.5)),
+    ("one_leaf", lambda: I.random_cloud(500, seed=12, leaf_size=2000, batch_size=2000)),
+    ("theta0", lambda: I.random_cloud(2000, seed=13, leaf_size=100, batch_size=100, theta=0.0)),
+]
+
+
+@pytest.mark.parametrize("name,make", CASES, ids=[c[0] for c in CASES])
+def test_host_plan_is_structurally_identical_to_oracle_tree(oracle_mod, name, make):
+    # R18: the 1e-12 GPU-vs-CPU parity is defined for structurally identical trees -> compare first.
+    c = make()
+    p = B.bltc_create_host_plan(None, c.coords(), None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    e = B.bltc_export_plan(p)
+    st = B.bltc_get_stats(p)
+    op = oracle_mod.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    oe = op.export()
+    for key in e:                                            # integer-exact permutation/ranges/lists, bitwise boxes
+        np.testing.assert_array_equal(e[key], oe[key], err_msg=key)
+    assert (st["n_clusters"], st["n_leaves"], st["n_batches"]) == (op.n_clusters, op.n_leaves, op.n_batches)
+    assert (st["far_evals"], st["near_evals"]) == (op.far_evals, op.near_evals)
+    assert st["shared_batches"] == op.shared_batches
+    B.bltc_destroy(p)
+
+
+def test_host_plan_separate_targets(oracle_mod):
+    c = I.random_cloud(3000, seed=10, leaf_size=200, batch_size=200, degree=4)
+    rng = np.random.default_rng(12)
+    T = np.ascontiguousarray(rng.random((3, c.N)))
+    p = B.bltc_create_host_plan(T, c.coords(), None, c.N, 0.7, 4, 200, 200)
+    e = B.bltc_export_plan(p)
+    oe = oracle_mod.OraclePlan((c.x, c.y, c.z), 0.7, 4, 200, 200, targets=(T[0], T[1], T[2])).export()
+    for key in e:
+        np.testing.assert_array_equal(e[key], oe[key], err_msg=key)
+    assert B.bltc_get_stats(p)["shared_batches"] == 0
