@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200 BLTC Yukawa convolution (BASELINE.json metric).
+
+  python bench.py --gpus N --steps K --warmup W            our CUDA path (one rank per GPU)
+  python bench.py --impl reference --steps K --warmup W     the CPU oracle, as it stands, on host cores
+
+A "step" is one pass of the whole hot path: one bltc_convolve call for all
+orbitals of the workload = BASELINE.json configs[1] (Be-like atom, adaptive Fejer mesh, 2 orbitals,
+theta 0.7, degree 8, N_L = N_B = 2000).  The plan (a0, host tree build) is built once before the
+timed region and reported separately, as the paper does (stage 1 vs stage 2).
+
+value   = equivalent direct interactions per second = n_orb * N^2 * n_gpus / t_step (inputs in HBM)
+e2e     = the same through the C ABI with HOST (pinned) buffers: H2D of f and D2H of out inside the
+          timed region
+roofline= FP64 ALU bound: executed FP64 flops of the dominant kernel / its CUDA-event time / FP64 peak
+Multi-GPU: the path does not need to shard on one node ("replicas only"): every rank runs
+the same convolution on its own GPU (weak scaling), no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "fp64 BLTC convolution, equivalent direct interactions/s"
+UNIT = "interactions/s"
+
+# FP64 instruction mix of one kernel evaluation, counted in the SASS of the inner loops
+# (profiles/r01_sass_counts.md).  flops = 2*DFMA + DMUL + DADD.
+# key: (kernel, orbital tile width OT) -> flops per (target, source/proxy point) pair for ALL OT orbitals
+FLOPS_PER_PAIR = {
+    ("near", 1): 41.0, ("near", 2): 64.0, ("near", 3): 87.0, ("near", 4): 110.0,
+    ("far", 1): 36.0, ("far", 2): 60.0, ("far", 3): 84.0, ("far", 4): 108.0,
+}
+# 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
+# probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.
+FP64_PEAK_TFLOPS_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def orbital_groups(n_orb, max_ot=4):
+    ng = (n_orb + max_ot - 1) // max_ot
+    g = [n_orb // ng] * ng
+    for i in range(n_orb % ng):
+        g[i] += 1
+    return g
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            p = [x.strip() for x in r.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1])); pw.append(float(p[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload():
+    from paper_2003_01833_b200 import inputs as I
+    return I.config1()
+
+
+def cpu_oracle_sample(c, batches, repeat=1):
+    """Time the CPU oracle's BLTC (as it stands) on a bounded sample of target batches and scale to the
+    whole convolution by evaluation count.  Returns (equiv. interactions/s, seconds, description)."""
+    import oracle
+    op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    e = op.export()
+    size = e["cl_end"] - e["cl_begin"]
+    ev = 0
+    for b in batches:
+        nt = e["b_end"][b] - e["b_begin"][b]
+        ev += nt * (op.P * (e["far_ptr"][b + 1] - e["far_ptr"][b])
+                    + size[e["near_idx"][e["near_ptr"][b]:e["near_ptr"][b + 1]]].sum())
+    total = op.far_evals + op.near_evals
+    best = None
+    for _ in range(repeat):
+        t0 = time.perf_counter()
+        op.evaluate(c.w, c.f, c.k, batches=list(batches))
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    t_full = best * total / ev                       # seconds for all batches, all orbitals
+    value = c.n_orb * float(c.N) ** 2 / t_full
+    ntg = int(sum(e["b_end"][b] - e["b_begin"][b] for b in batches))
+    desc = (f"CPU BLTC oracle (oracle/bltc_cpu.c, strict IEEE, long-double sums) on {len(batches)} of "
+            f"{op.n_batches} target batches ({ntg} targets, {c.n_orb} orbitals, {ev * c.n_orb:.3g} kernel "
+            f"evaluations incl. their proxy charges), {best:.2f} s, scaled by evaluation count to the "
+            f"whole convolution")
+    return value, best, desc, oracle.n_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    c = workload()
+    batches = [137]
+    vals = []
+    for i in range(args.warmup + args.steps):
+        v, dt, desc, cores = cpu_oracle_sample(c, batches)
+        if i >= args.warmup:
+            vals.append((v, dt))
+    value = float(np.mean([v for v, _ in vals]))
+    ms = float(np.mean([dt for _, dt in vals])) * 1e3
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": c.name, "N": c.N, "n_orb": c.n_orb, "theta": c.theta, "degree": c.degree,
+                   "leaf_size": c.leaf_size, "batch_size": c.batch_size,
+                   "note": "each step = the CPU oracle on a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2003_01833_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+
+    c = workload()
+    N, O = c.N, c.n_orb
+    X = torch.from_numpy(c.coords()).cuda()
+    w = torch.from_numpy(c.w).cuda()
+    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+    out = torch.empty((O, N), dtype=torch.float64, device="cuda")
+    t0 = time.perf_counter()
+    plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    create_ms = (time.perf_counter() - t0) * 1e3
+    st = B.bltc_get_stats(plan)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    groups = orbital_groups(O)
+    launches_per_step = 5 * len(groups)
+
+    # ---- device-resident timing -------------------------------------------------------------
+    B.bltc_set_profiling(plan, True)
+    for _ in range(max(args.warmup, 3)):
+        B.bltc_convolve(plan, c.k, f, O, out, True)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    phase_sum = {p: 0.0 for p in B.PHASES}
+    barrier()
+    for i in range(args.steps):
+        flush.fill_(0.0)                                        # L2 flush between timed iterations
+        ev[i][0].record(stream)
+        B.bltc_convolve(plan, c.k, f, O, out, True)
+        ev[i][1].record(stream)
+        ph = B.bltc_get_phase_ms(plan)                          # syncs on the step's last event
+        for p in B.PHASES:
+            phase_sum[p] += ph[p]
+    barrier()
+    clocks = sampler.stop()
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if world > 1:
+        t = torch.tensor([t_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_ms = float(t.item())
+    ms_per_step = t_ms / args.steps
+    value = world * O * float(N) ** 2 / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers ------------------------------------
+    B.bltc_set_profiling(plan, False)
+    f_host = torch.from_numpy(np.ascontiguousarray(c.f)).pin_memory()
+    out_host = torch.empty((O, N), dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        B.bltc_convolve(plan, c.k, f_host, O, out_host, True)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_ms = 0.0
+    for i in range(args.steps):
+        flush.fill_(0.0)
+        e0.record(stream)
+        B.bltc_convolve(plan, c.k, f_host, O, out_host, True)   # H2D(f) + a1..a5 + D2H(out) + stream sync
+        e1.record(stream)
+        e1.synchronize()
+        e2e_ms += e0.elapsed_time(e1)
+    barrier()
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = world * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
+    same = bool(np.array_equal(out_host.numpy(), out.cpu().numpy()))
+
+    if rank == 0:
+        near_ms = phase_sum["near"] / args.steps / len(groups)      # average launch duration
+        far_ms = phase_sum["far"] / args.steps / len(groups)
+        near_flops = sum(st["near_evals"] * FLOPS_PER_PAIR[("near", g)] for g in groups) / len(groups)
+        far_flops = sum(st["far_evals"] * FLOPS_PER_PAIR[("far", g)] for g in groups) / len(groups)
+        peak = FP64_PEAK_TFLOPS_NOMINAL
+        near_tf = near_flops / (near_ms * 1e-3) / 1e12
+        far_tf = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
+        probe = B.bltc_probe_fp64(64)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "r01_near_traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+            except Exception:
+                traffic = None
+        cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, [0, 137, 301, 567])
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c.name + " (BASELINE.json configs[1])", "N": N, "n_orb": O, "theta": c.theta,
+                       "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
+                       "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "time_per_convolution_ms": ms_per_step / O,
+            "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O / (ms_per_step * 1e-3),
+            "phase_ms": {p: phase_sum[p] / args.steps for p in B.PHASES},
+            "plan": {"create_ms": create_ms, "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
+                     "clusters": st["n_clusters"], "batches": st["n_batches"],
+                     "far_evals": st["far_evals"], "near_evals": st["near_evals"]},
+            "roofline": {"bound": "alu", "kernel": "near_kernel", "achieved": near_tf, "peak": peak,
+                         "unit": "TFLOP/s", "frac": near_tf / peak, "traffic": traffic,
+                         "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "peak_measured_dfma_probe": probe, "avg_launch_ms": near_ms,
+                         "flops_per_launch": near_flops},
+            "roofline_far": {"bound": "alu", "kernel": "far_kernel", "achieved": far_tf, "peak": peak,
+                             "unit": "TFLOP/s", "frac": far_tf / peak, "avg_launch_ms": far_ms,
+                             "flops_per_launch": far_flops},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": O * N * 8,
+                    "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_ms / args.steps,
+                    "bitwise_equal_to_device_path": same},
+            "gpu_launches": launches_per_step * args.steps,
+            "clocks": clocks,
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},
+        }
+        print(json.dumps(line))
+    B.bltc_destroy(plan)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
