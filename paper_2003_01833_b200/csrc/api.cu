@@ -411,8 +411,7 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
     for (size_t g = 0; g < groups.size(); ++g) {
         const int ot = groups[g];
         const int rv = targets_per_thread(ot) - 1;
-        KNeg nk;
-        for (int o = 0; o < kMaxOT; ++o) nk.nk[o] = o < ot ? -k[o0 + o] : -1.0;
+        const KPar nk = make_kpar(k + o0, ot);
         cudaEvent_t* ev = h->profiling ? &h->events[g * per] : nullptr;
         if (ev) BLTC_CUDA(cudaEventRecord(ev[0], st));
         // a1: gather to tree order
@@ -564,8 +563,7 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
         const int rv = targets_per_thread(ot) - 1;
         if (!t_items[rv].p)
             BLTC_CUDA(put(t_items[rv], items[rv].data(), items[rv].size() * sizeof(WorkItem)));
-        KNeg nk;
-        for (int o = 0; o < kMaxOT; ++o) nk.nk[o] = o < ot ? -k[o0 + o] : -1.0;
+        const KPar nk = make_kpar(k + o0, ot);
         BLTC_CUDA(launch_gather(d_fs, N, o0, ot, nullptr, N, t_fsrc.as<double>(), st));
         if (sub) BLTC_CUDA(launch_gather(d_ft, M, o0, ot, nullptr, M, t_ftgt.as<double>(), st));
         cudaEvent_t ea = nullptr, eb = nullptr;

@@ -1,46 +1,62 @@
 // fp64_math.cuh -- branch-free FP64 rsqrt and exp(x <= 0) for the Yukawa kernel
 //   G_k(r) = exp(-k r) / (4 pi r)        (Eq. (18), north_star)
-// tuned for the sm_100a FP64 pipe (64 lanes/SM: one warp-wide DFMA per 2 cycles per SM
-// sub-partition, so every non-FP64 instruction -- MUFU seed, LDS table look-up, integer
-// exponent insertion -- issues in the FP64 pipe's shadow and is free).
+// tuned for the sm_100a FP64 pipe: 64 lanes/SM, one warp-wide FP64 instruction per 2 cycles per SM
+// sub-partition.  Measured on B200: step time ~ 2 x (FP64 instructions) +
+// (non-FP64 instructions that do not land in the shadow cycle of an FP64 issue), and FMA-pipe
+// instructions (IMAD, IMAD.MOV, IMAD.SHL) cost the FP64 pipe 1-2 cycles each.  So both functions
+// minimise the FP64 count AND keep their integer work on the ALU pipe (SHF / LOP3 / ISETP / SEL via
+// inline PTX that ptxas cannot turn into IMAD).
 //
-// Accuracy target: <= ~1.5 ulp per kernel value (the parity tolerances are 1e-13 / 1e-12
-// relative 2-norm on sums of 1e4..1e6 terms).
-//
-//   rsqrt: MUFU.RSQ64H seed (rel. error <~ 2^-20) + one cubic (Halley-type) step,
-//          5 FP64 instructions, residual 5 e^3/16 < 2^-58.
-//   exp:   x = 16 n' ... exp(x) = 2^n * 2^(j/16) * p(r),  n16 = rint(x * 16/ln2) = 16 n + j,
-//          r = x - n16 ln2/16, |r| <= ln2/32, p = degree-6 near-minimax polynomial
-//          (max rel. error 7.6e-18 in exact arithmetic), 2^(j/16) from a 16-entry shared-memory
-//          table (16 x 8 B = 32 banks: conflict-free), 2^n by integer add into the exponent field.
-//          4 + 6 + 1 = 11 FP64 instructions.  Argument must satisfy -2^30 < x <= 0 (x = -k r);
-//          results below 2^-1022 are clamped to ~2^-1022 (absolute error < 1e-307).
-//   Coefficients: Chebyshev-node interpolant of exp on [-ln2/32, ln2/32] computed in 60-digit
-//   arithmetic and rounded to double; T16[j] = 2^(j/16) correctly rounded.
+//   rsqrt: MUFU.RSQ64H seed (XU pipe, rel. error <~ 2^-20) + one cubic step: 5 FP64 instructions,
+//          residual 5 e^3/16 < 2^-58; +1 for r = r2 * rinv.
+//   exp:   u = r * c,  c = -k T/ln2 (per orbital, host-computed),  T = 2048;
+//          t = u + (1.5*2^52 + 1023 T)  ->  low word m = rint(u) + 1023 T = T*(n + 1023) + j
+//          rho = u - rint(u) in [-1/2, 1/2];   exp(-k r) = 2^n * 2^(j/T) * (1 + rho (C1 + C2 rho + C3 rho^2))
+//          2^(j/T): 16 KB shared-memory table (bank conflicts are harmless here: measured);
+//          2^n: the biased exponent n + 1023 = m >> 11 is merged into the table value's exponent field
+//          with one rotate + one LOP3 (the table values are in [1,2), exponent field 0x3FF).
+//          7 FP64 instructions.  Polynomial error 8.6e-18, total <= ~1 ulp.
+//          Any u <= 0 is legal: if m < 0 (exp(-k r) < 2^-1023) the high word of t differs from 0x43380000
+//          and m is replaced by 0, which gives a subnormal-sized value (absolute error < 1e-307).
 #pragma once
 #include <cuda_runtime.h>
+#include <cstdint>
+
+#include "exp_table.inc"
 
 namespace bltc {
 
-__device__ __constant__ const double kExpT16[16] = {
-    0x1.0000000000000p+0, 0x1.0b5586cf9890fp+0, 0x1.172b83c7d517bp+0, 0x1.2387a6e756238p+0,
-    0x1.306fe0a31b715p+0, 0x1.3dea64c123422p+0, 0x1.4bfdad5362a27p+0, 0x1.5ab07dd485429p+0,
-    0x1.6a09e667f3bcdp+0, 0x1.7a11473eb0187p+0, 0x1.8ace5422aa0dbp+0, 0x1.9c49182a3f090p+0,
-    0x1.ae89f995ad3adp+0, 0x1.c199bdd85529cp+0, 0x1.d5818dcfba487p+0, 0x1.ea4afa2a490dap+0};
+constexpr int kExpT = BLTC_EXP_T;
+constexpr int kExpLog2T = BLTC_EXP_LOG2T;
+constexpr int kExpTableBytes = kExpT * 8;
+constexpr double kExpMagic = 6755399441055744.0 + 1023.0 * BLTC_EXP_T;   // 1.5 * 2^52 + 1023 T (exact)
 
-#define BLTC_EXP_16_OVER_LN2 0x1.71547652b82fep+4
-#define BLTC_EXP_LN2_OVER_16 0x1.62e42fefa39efp-5
-#define BLTC_EXP_MAGIC 6755399441055744.0 /* 1.5 * 2^52 */
-#define BLTC_EXP_C1 0x1.000000000000ap+0
-#define BLTC_EXP_C2 0x1.0000000000003p-1
-#define BLTC_EXP_C3 0x1.5555555405047p-3
-#define BLTC_EXP_C4 0x1.55555554ad2d0p-5
-#define BLTC_EXP_C5 0x1.11126efea4abcp-7
-#define BLTC_EXP_C6 0x1.6c181f5984fddp-10
+__device__ const double kExpTab[BLTC_EXP_T] = {BLTC_EXP_TABLE};
 
-// Copy the table to shared memory (call from the first 16 threads, then __syncthreads()).
-__device__ __forceinline__ void exp_table_init(double* t16_smem, int tid) {
-    if (tid < 16) t16_smem[tid] = kExpT16[tid];
+// Shared-memory table: the caller provides >= 2 * kExpTableBytes of dynamic shared memory at `raw`
+// (shared-window byte address); the table is placed at the next multiple of kExpTableBytes so that
+// "base | offset" addresses it.  Call with all threads, then __syncthreads().
+__device__ __forceinline__ uint32_t exp_table_init(uint32_t raw, int tid, int nthreads) {
+    const uint32_t base = (raw + kExpTableBytes - 1) & ~(uint32_t)(kExpTableBytes - 1);
+    for (int i = tid; i < kExpT; i += nthreads) {
+        const double v = kExpTab[i];
+        asm volatile("st.shared.f64 [%0], %1;" ::"r"(base + 8u * i), "d"(v));
+    }
+    return base;
+}
+
+// Constants that must live in registers (an FP64 instruction takes at most one non-register operand;
+// without this ptxas re-materialises them with IMAD.MOV inside the loop).  Loaded once per thread
+// from values the compiler cannot see through.
+struct MathRegs {
+    double c375;    // 0.375
+    double c2;      // BLTC_EXP_C2
+};
+__device__ __forceinline__ MathRegs math_regs_init(const double* __restrict__ opaque2) {
+    MathRegs m;
+    m.c375 = opaque2[0];
+    m.c2 = opaque2[1];
+    return m;
 }
 
 // MUFU.RSQ64H: approximate 1/sqrt from the high word only.
@@ -53,37 +69,42 @@ __device__ __forceinline__ double rsqrt_seed(double x) {
 // rinv = 1/sqrt(r2), r = sqrt(r2).  ZERO_SAFE: r2 == 0 gives rinv = 0, r = 0 (the singular
 // term "is skipped") via one integer compare + select on the seed's high word.
 template <bool ZERO_SAFE>
-__device__ __forceinline__ void rsqrt_sqrt(double r2, double& rinv, double& r) {
-    double y0 = rsqrt_seed(r2);
-    if (ZERO_SAFE) {
-        int hi = __double2hiint(y0);
-        hi = (hi == 0x7ff00000) ? 0 : hi;          // +inf (r2 == 0)  ->  +0
-        y0 = __hiloint2double(hi, __double2loint(y0));
-    }
-    double t = r2 * y0;                 // ~ sqrt(r2)
-    double e = fma(-t, y0, 1.0);        // 1 - r2 y0^2
-    double p = fma(0.375, e, 0.5);
-    double ye = y0 * e;
-    rinv = fma(ye, p, y0);              // y0 (1 + e/2 + 3 e^2/8)
+__device__ __forceinline__ void rsqrt_sqrt(double r2, double& rinv, double& r, const MathRegs& mr) {
+    int hi = __double2hiint(rsqrt_seed(r2));
+    if (ZERO_SAFE) hi = (hi == 0x7ff00000) ? 0 : hi;     // +inf (r2 == 0)  ->  +0
+    uint32_t lo;
+    asm("shr.u32 %0, %1, 31;" : "=r"(lo) : "r"(hi));     // = 0 (the seed is positive); an ALU-pipe "mov"
+    const double y0 = __hiloint2double(hi, (int)lo);
+    const double t = r2 * y0;                 // ~ sqrt(r2)
+    const double e = fma(-t, y0, 1.0);        // 1 - r2 y0^2
+    const double p = fma(e, mr.c375, 0.5);
+    const double ye = y0 * e;
+    rinv = fma(ye, p, y0);                    // y0 (1 + e/2 + 3 e^2/8)
     r = r2 * rinv;
 }
 
-// exp(x) for -2^30 < x <= 0.  t16: shared-memory copy of kExpT16.
-__device__ __forceinline__ double exp_neg(double x, const double* __restrict__ t16) {
-    double t = fma(x, BLTC_EXP_16_OVER_LN2, BLTC_EXP_MAGIC);
-    int n16 = __double2loint(t);                    // rint(x * 16/ln2), two's complement
-    double nf = t - BLTC_EXP_MAGIC;
-    double r = fma(nf, -BLTC_EXP_LN2_OVER_16, x);
-    double tj = t16[n16 & 15];
-    double p = fma(BLTC_EXP_C6, r, BLTC_EXP_C5);
-    p = fma(p, r, BLTC_EXP_C4);
-    p = fma(p, r, BLTC_EXP_C3);
-    p = fma(p, r, BLTC_EXP_C2);
-    p = fma(p, r, BLTC_EXP_C1);
-    double s = tj * r;
-    double e = fma(s, p, tj);                       // tj * (1 + r p(r))
-    int n = max(n16 >> 4, -1022);                   // clamp: result stays a normal number
-    return __hiloint2double(__double2hiint(e) + (n << 20), __double2loint(e));
+// exp(-k r) given r >= 0 and c = -k T/ln2.  tab = value returned by exp_table_init.
+__device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, const MathRegs& mr) {
+    const double t = fma(r, c, kExpMagic);
+    const double nf = t - kExpMagic;                    // rint(u), exact
+    const double rho = fma(r, c, -nf);
+    const int m = (__double2hiint(t) == 0x43380000) ? __double2loint(t) : 0;
+    uint32_t r3, adr, lo, hi, rx, hi2;
+    asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(adr) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8), "r"(tab));   // (a & b) | c
+    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(adr));
+    asm("shf.l.wrap.b32 %0, %1, %1, %2;" : "=r"(rx) : "r"(m), "n"(20 - BLTC_EXP_LOG2T));
+    asm("lop3.b32 %0, %1, %2, %3, 0xE2;" : "=r"(hi2) : "r"(rx), "n"(0x7FF00000), "r"(hi));              // (a & b) | (c & ~b)
+    const double tj = __hiloint2double((int)hi2, (int)lo);   // 2^n * 2^(j/T)
+    double p = fma(rho, BLTC_EXP_C3, mr.c2);
+    p = fma(p, rho, BLTC_EXP_C1);
+    const double s = tj * rho;
+    return fma(s, p, tj);                               // tj (1 + rho p(rho))
+}
+
+// host side: c = -k T / ln2, rounded once from extended precision
+inline double exp_scale_of_k(double k) {
+    return (double)(-(long double)k * (long double)BLTC_EXP_T / 0.693147180559945309417232121458176568L);
 }
 
 }  // namespace bltc

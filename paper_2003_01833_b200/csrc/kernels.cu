@@ -25,6 +25,9 @@ namespace {
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
+// {0.375, BLTC_EXP_C2}: constants the pair kernels keep in registers (see fp64_math.cuh, MathRegs)
+__device__ double kMathOpaque[2] = {0.375, BLTC_EXP_C2};
+
 // ------------------------------------------------------------------------------------ a1 / pack
 __global__ void gather_kernel(const double* __restrict__ f, int64_t stride, int o0, int ot,
                               const int32_t* __restrict__ perm, int64_t n, double* __restrict__ dst) {
@@ -218,17 +221,18 @@ template <int R, int OT, bool SUB>
 __global__ void __launch_bounds__(kThreads, 2)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
-            const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KNeg nk,
+            const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
             double* __restrict__ partial, int64_t partial_len) {
-    __shared__ double4 s_rec[kSrcTile];
-    __shared__ double s_f[kSrcTile * OT];
-    __shared__ double s_t16[16];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     static_assert(sizeof(double4) * kSrcTile >= sizeof(double) * R * OT * 8 * 32, "reduction scratch");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
+    double4* s_rec = reinterpret_cast<double4*>(smem_raw + 2 * kExpTableBytes);
+    double* s_f = reinterpret_cast<double*>(s_rec + kSrcTile);
+    const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, S = 8 >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
-    exp_table_init(s_t16, tid);
     TargetRegs<R, OT> T;
     load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
 
@@ -260,11 +264,11 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
                 const double dx = T.x[r] - s.x, dy = T.y[r] - s.y, dz = T.z[r] - s.z;
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                 double rinv, rr;
-                rsqrt_sqrt<true>(r2, rinv, rr);            // r2 == 0: rinv = 0, the term vanishes
+                rsqrt_sqrt<true>(r2, rinv, rr, mr);        // r2 == 0: rinv = 0, the term vanishes
                 const double gw = rinv * s.w;
 #pragma unroll
                 for (int o = 0; o < OT; ++o) {
-                    const double ex = exp_neg(nk.nk[o] * rr, s_t16);
+                    const double ex = exp_neg_kr(rr, kp.c[o], tab, mr);
                     const double g = ex * gw;
                     const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
                     T.acc[r][o] = fma(g, df, T.acc[r][o]);
@@ -281,18 +285,19 @@ __global__ void __launch_bounds__(kThreads, 2)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
            const double* __restrict__ fhat, int n1, const double4* __restrict__ tgt_rec,
-           const double* __restrict__ ftgt, const KNeg nk, double* __restrict__ partial,
+           const double* __restrict__ ftgt, const KPar kp, double* __restrict__ partial,
            int64_t partial_len) {
-    __shared__ double s_w[kProxyTile];
-    __shared__ double s_fh[kProxyTile * OT];
-    __shared__ double s_nodes[3 * 21];
-    __shared__ double s_t16[16];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     static_assert(kProxyTile >= R * 8 * 32, "reduction scratch fits in s_fh");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
+    double* s_w = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
+    double* s_fh = s_w + kProxyTile;
+    double* s_nodes = s_fh + kProxyTile * OT;            // [3][21]
+    const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, S = 8 >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
-    exp_table_init(s_t16, tid);
     TargetRegs<R, OT> T;
     load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
 
@@ -336,10 +341,10 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
                         const double dz = T.z[r] - sz;
                         const double r2 = fma(dz, dz, dxy2[r]);
                         double rinv, rr;
-                        rsqrt_sqrt<false>(r2, rinv, rr);   // MAC keeps targets off the grid (theta < 1)
+                        rsqrt_sqrt<false>(r2, rinv, rr, mr);   // MAC keeps targets off the grid (theta < 1)
 #pragma unroll
                         for (int o = 0; o < OT; ++o) {
-                            const double ex = exp_neg(nk.nk[o] * rr, s_t16);
+                            const double ex = exp_neg_kr(rr, kp.c[o], tab, mr);
                             const double g = ex * rinv;
                             // fhat_k - f_i what_k: interpolated charges of (f_j - f_i) w_j (reading R11)
                             const double qk = SUB ? fma(-T.f[r][o], wv, fv[o]) : fv[o];
@@ -359,7 +364,7 @@ __global__ void __launch_bounds__(kThreads)
 epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__ b_count,
                 const int64_t* __restrict__ b_partial_base, const int32_t* __restrict__ b_nseg,
                 const double* __restrict__ partial, int64_t partial_len, const double* __restrict__ ftgt,
-                const KNeg nk, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
+                const KPar kp, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
                 int o0) {
     const int b = blockIdx.x;
     const int begin = b_begin[b], count = b_count[b], nseg = b_nseg[b];
@@ -372,7 +377,7 @@ epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__
             double s = 0.0;
             for (int g = 0; g < nseg; ++g) s += partial[(int64_t)o * partial_len + base + (int64_t)g * count + l];
             double v = -kInv2Pi * s;                               // -2 * S / (4 pi)
-            if (SUB) v = fma(-2.0 / (nk.nk[o] * nk.nk[o]), ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2
+            if (SUB) v = fma(-2.0 / (kp.nk[o] * kp.nk[o]), ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2
             out[(int64_t)(o0 + o) * stride + dst] = v;
         }
     }
@@ -397,6 +402,9 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
+size_t near_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + kSrcTile * (sizeof(double4) + sizeof(double) * ot); }
+size_t far_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + sizeof(double) * (kProxyTile * (1 + (size_t)ot) + 3 * 21); }
+
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {
     if (bytes > 48 * 1024) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -406,6 +414,16 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 }  // namespace
 
 // ===================================================================================== launchers
+KPar make_kpar(const double* k, int ot) {
+    KPar kp;
+    for (int o = 0; o < kMaxOT; ++o) {
+        const double kk = o < ot ? k[o] : 1.0;
+        kp.nk[o] = -kk;
+        kp.c[o] = exp_scale_of_k(kk);
+    }
+    return kp;
+}
+
 cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
                           int64_t n, double* dst, cudaStream_t st) {
     if (n == 0) return cudaSuccess;
@@ -445,15 +463,26 @@ cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const in
 
 cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
-                       const double4* tgt_rec, const double* ftgt, const KNeg& nk, double* partial,
+                       const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
     const int n1 = degree + 1;
+    cudaError_t e = cudaSuccess;
 #define BLTC_FAR(RV, OTV)                                                                               \
-    if (subtract) far_kernel<RV, OTV, true><<<nitems, kThreads, 0, st>>>(items, far_slots, slot_nodes,  \
-        what, fhat, n1, tgt_rec, ftgt, nk, partial, partial_len);                                       \
-    else far_kernel<RV, OTV, false><<<nitems, kThreads, 0, st>>>(items, far_slots, slot_nodes, what,    \
-        fhat, n1, tgt_rec, ftgt, nk, partial, partial_len);
+    {                                                                                                   \
+        const size_t smem = far_smem_bytes(OTV);                                                        \
+        if (subtract) {                                                                                 \
+            e = set_smem(far_kernel<RV, OTV, true>, smem);                                              \
+            if (e != cudaSuccess) return e;                                                             \
+            far_kernel<RV, OTV, true><<<nitems, kThreads, smem, st>>>(items, far_slots, slot_nodes,     \
+                what, fhat, n1, tgt_rec, ftgt, kp, partial, partial_len);                               \
+        } else {                                                                                        \
+            e = set_smem(far_kernel<RV, OTV, false>, smem);                                             \
+            if (e != cudaSuccess) return e;                                                             \
+            far_kernel<RV, OTV, false><<<nitems, kThreads, smem, st>>>(items, far_slots, slot_nodes,    \
+                what, fhat, n1, tgt_rec, ftgt, kp, partial, partial_len);                               \
+        }                                                                                               \
+    }
     switch (ot) {
         case 1: BLTC_FAR(2, 1) break;
         case 2: BLTC_FAR(2, 2) break;
@@ -467,14 +496,25 @@ cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems,
 
 cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
-                        const double* ftgt, const KNeg& nk, double* partial, int64_t partial_len,
+                        const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
+    cudaError_t e = cudaSuccess;
 #define BLTC_NEAR(RV, OTV)                                                                              \
-    if (subtract) near_kernel<RV, OTV, true><<<nitems, kThreads, 0, st>>>(items, ranges, src_rec, fsrc, \
-        tgt_rec, ftgt, nk, partial, partial_len);                                                       \
-    else near_kernel<RV, OTV, false><<<nitems, kThreads, 0, st>>>(items, ranges, src_rec, fsrc,         \
-        tgt_rec, ftgt, nk, partial, partial_len);
+    {                                                                                                   \
+        const size_t smem = near_smem_bytes(OTV);                                                       \
+        if (subtract) {                                                                                 \
+            e = set_smem(near_kernel<RV, OTV, true>, smem);                                             \
+            if (e != cudaSuccess) return e;                                                             \
+            near_kernel<RV, OTV, true><<<nitems, kThreads, smem, st>>>(items, ranges, src_rec, fsrc,    \
+                tgt_rec, ftgt, kp, partial, partial_len);                                               \
+        } else {                                                                                        \
+            e = set_smem(near_kernel<RV, OTV, false>, smem);                                            \
+            if (e != cudaSuccess) return e;                                                             \
+            near_kernel<RV, OTV, false><<<nitems, kThreads, smem, st>>>(items, ranges, src_rec, fsrc,   \
+                tgt_rec, ftgt, kp, partial, partial_len);                                               \
+        }                                                                                               \
+    }
     switch (ot) {
         case 1: BLTC_NEAR(2, 1) break;
         case 2: BLTC_NEAR(2, 2) break;
@@ -488,15 +528,15 @@ cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems
 
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
-                            int64_t partial_len, const double* ftgt, const KNeg& nk, const int32_t* perm,
+                            int64_t partial_len, const double* ftgt, const KPar& kp, const int32_t* perm,
                             double* out, int64_t stride, int o0, cudaStream_t st) {
     if (nbatch == 0) return cudaSuccess;
 #define BLTC_EPI(OTV)                                                                                  \
     case OTV:                                                                                          \
         if (subtract) epilogue_kernel<OTV, true><<<nbatch, kThreads, 0, st>>>(b_begin, b_count,        \
-            b_partial_base, b_nseg, partial, partial_len, ftgt, nk, perm, out, stride, o0);            \
+            b_partial_base, b_nseg, partial, partial_len, ftgt, kp, perm, out, stride, o0);            \
         else epilogue_kernel<OTV, false><<<nbatch, kThreads, 0, st>>>(b_begin, b_count,                \
-            b_partial_base, b_nseg, partial, partial_len, ftgt, nk, perm, out, stride, o0);            \
+            b_partial_base, b_nseg, partial, partial_len, ftgt, kp, perm, out, stride, o0);            \
         break;
     switch (ot) {
         BLTC_EPI(1) BLTC_EPI(2) BLTC_EPI(3) BLTC_EPI(4)

@@ -15,7 +15,10 @@ constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile
 // targets per thread for an orbital tile of width ot
 inline int targets_per_thread(int ot) { return ot <= 2 ? 2 : 1; }
 
-struct KNeg { double nk[kMaxOT]; };    // -k_o of the orbital tile (kernel parameter -> constant bank)
+// per-orbital constants of the tile (kernel parameter -> constant bank):
+//   nk = -k_o;  c = -k_o T/ln2 (scaled exponent argument of fp64_math.cuh's exp)
+struct KPar { double nk[kMaxOT]; double c[kMaxOT]; };
+KPar make_kpar(const double* k, int ot);   // k: ot values (host)
 
 // a1: f[o0+o][perm[i]] -> dst[i][ot] (tree order, orbital-interleaved)
 cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
@@ -33,19 +36,19 @@ cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const in
 // a3: far field
 cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
-                       const double4* tgt_rec, const double* ftgt, const KNeg& nk, double* partial,
+                       const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st);
 
 // a4 / a6: near field and brute-force direct sum (same kernel, different work items)
 cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
-                        const double* ftgt, const KNeg& nk, double* partial, int64_t partial_len,
+                        const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st);
 
 // a5: out[o0+o][perm[i]] = -2 ( (far + near)/(4 pi) + [subtract] f_i / k_o^2 )
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
-                            int64_t partial_len, const double* ftgt, const KNeg& nk, const int32_t* perm,
+                            int64_t partial_len, const double* ftgt, const KPar& kp, const int32_t* perm,
                             double* out, int64_t stride, int o0, cudaStream_t st);
 
 // roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed
