@@ -36,11 +36,11 @@ METRIC = "fp64 BLTC convolution, equivalent direct interactions/s"
 UNIT = "interactions/s"
 
 # FP64 instruction mix of one kernel evaluation, counted in the SASS of the inner loops
-# (profiles/r01_sass_counts.md).  flops = 2*DFMA + DMUL + DADD.
+# (profiles/r01*_sass_counts.md; tests/test_library_host.py re-counts them from the built library).  flops = 2*DFMA + DMUL + DADD.
 # key: (kernel, orbital tile width OT) -> flops per (target, source/proxy point) pair for ALL OT orbitals
 FLOPS_PER_PAIR = {
-    ("near", 1): 41.0, ("near", 2): 64.0, ("near", 3): 87.0, ("near", 4): 110.0,
-    ("far", 1): 36.0, ("far", 2): 60.0, ("far", 3): 84.0, ("far", 4): 108.0,
+    ("near", 1): 34.0, ("near", 2): 50.0, ("near", 3): 66.0, ("near", 4): 82.0,
+    ("far", 1): 29.0, ("far", 2): 46.0, ("far", 3): 63.0, ("far", 4): 80.0,
 }
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.

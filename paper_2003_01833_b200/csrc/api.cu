@@ -3,6 +3,7 @@
 // method lives here; it is all in kernels.cu (device) and plan_host.cpp (tree and lists).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <chrono>
 #include <cmath>
 #include <cstring>
@@ -412,6 +413,10 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
         const int ot = groups[g];
         const int rv = targets_per_thread(ot) - 1;
         const KPar nk = make_kpar(k + o0, ot);
+        // exp underflow guard: not needed when k r < 700 for every pair (max_dist bounds r)
+        double kmax = 0.0;
+        for (int o = 0; o < ot; ++o) kmax = std::max(kmax, k[o0 + o]);
+        const bool guard = !(kmax * hp.max_dist < 700.0);
         cudaEvent_t* ev = h->profiling ? &h->events[g * per] : nullptr;
         if (ev) BLTC_CUDA(cudaEventRecord(ev[0], st));
         // a1: gather to tree order
@@ -427,12 +432,12 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
                                 h->src_rec.p, h->fsrc.p, h->fhat.p, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
         // a3: far field
-        BLTC_CUDA(launch_far(ot, sub, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
+        BLTC_CUDA(launch_far(ot, sub, guard, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
                              h->slot_nodes.p, h->what.p, h->fhat.p, hp.degree, h->tgt_rec, ftgt, nk,
                              h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[3], st));
         // a4: near field
-        BLTC_CUDA(launch_near(ot, sub, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
+        BLTC_CUDA(launch_near(ot, sub, guard, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
                               h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
         // a5: epilogue
@@ -508,7 +513,7 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
         nsplit = (int)std::min<int64_t>(64, std::max<int64_t>(1, (want + tiles512 - 1) / tiles512));
         nsplit = (int)std::min<int64_t>(nsplit, std::max<int64_t>(1, N / 256));
         for (int s = 0; s < nsplit; ++s)
-            ranges.push_back(Range{(int32_t)(N * s / nsplit), (int32_t)(N * (s + 1) / nsplit)});
+            ranges.push_back(Range{(int32_t)(N * s / nsplit), (int32_t)(N * (s + 1) / nsplit), kRangeMayCoincide});
         for (int64_t b0 = 0; b0 < M; b0 += kPB) {
             pb_begin.push_back((int32_t)b0);
             pb_count.push_back((int32_t)std::min<int64_t>(kPB, M - b0));
@@ -571,7 +576,7 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
             BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
             BLTC_CUDA(cudaEventRecord(ea, st));
         }
-        BLTC_CUDA(launch_near(ot, sub, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
+        BLTC_CUDA(launch_near(ot, sub, true, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }

@@ -40,7 +40,14 @@ __device__ __forceinline__ uint32_t exp_table_init(uint32_t raw, int tid, int nt
     const uint32_t base = (raw + kExpTableBytes - 1) & ~(uint32_t)(kExpTableBytes - 1);
     for (int i = tid; i < kExpT; i += nthreads) {
         const double v = kExpTab[i];
-        asm volatile("st.shared.f64 [%0], %1;" ::"r"(base + 8u * i), "d"(v));
+        // entry j holds the mantissa of 2^(j/T) with the high word pre-biased by -(j << (20 - log2 T)):
+        // adding (m << (20 - log2 T)), m = T (n + 1023) + j, then yields 2^n 2^(j/T) with one shift-add
+#ifdef BLTC_X_LOPMERGE
+        const uint32_t hi = (uint32_t)__double2hiint(v);
+#else
+        const uint32_t hi = ((uint32_t)__double2hiint(v) & 0x000fffffu) - ((uint32_t)i << (20 - kExpLog2T));
+#endif
+        asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(base + 8u * i), "r"((uint32_t)__double2loint(v)), "r"(hi));
     }
     return base;
 }
@@ -51,11 +58,13 @@ __device__ __forceinline__ uint32_t exp_table_init(uint32_t raw, int tid, int nt
 struct MathRegs {
     double c375;    // 0.375
     double c2;      // BLTC_EXP_C2
+    double magic;   // kExpMagic
 };
-__device__ __forceinline__ MathRegs math_regs_init(const double* __restrict__ opaque2) {
+__device__ __forceinline__ MathRegs math_regs_init(const double* __restrict__ opaque3) {
     MathRegs m;
-    m.c375 = opaque2[0];
-    m.c2 = opaque2[1];
+    m.c375 = opaque3[0];
+    m.c2 = opaque3[1];
+    m.magic = opaque3[2];
     return m;
 }
 
@@ -78,28 +87,39 @@ __device__ __forceinline__ void rsqrt_sqrt(double r2, double& rinv, double& r, c
     const double t = r2 * y0;                 // ~ sqrt(r2)
     const double e = fma(-t, y0, 1.0);        // 1 - r2 y0^2
     const double p = fma(e, mr.c375, 0.5);
-    const double ye = y0 * e;
-    rinv = fma(ye, p, y0);                    // y0 (1 + e/2 + 3 e^2/8)
+    const double q = e * p;
+    rinv = fma(y0, q, y0);                    // y0 (1 + e/2 + 3 e^2/8); two distinct register operands
     r = r2 * rinv;
 }
 
 // exp(-k r) given r >= 0 and c = -k T/ln2.  tab = value returned by exp_table_init.
-__device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, const MathRegs& mr) {
-    const double t = fma(r, c, kExpMagic);
-    const double nf = t - kExpMagic;                    // rint(u), exact
+// GUARD = false is legal only when the caller has proved k r < 708 for every pair (no underflow);
+// ec = per-launch constants that live in uniform registers (kernel parameter).
+struct ExpConst { double c1, c3; };
+template <bool GUARD>
+__device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, const MathRegs& mr,
+                                             const ExpConst& ec) {
+    const double t = fma(r, c, mr.magic);
+    const double nf = t - mr.magic;                     // rint(u), exact
     const double rho = fma(r, c, -nf);
-    const int m = (__double2hiint(t) == 0x43380000) ? __double2loint(t) : 0;
-    uint32_t r3, adr, lo, hi, rx, hi2;
+    int m = __double2loint(t);
+    if (GUARD) m = (__double2hiint(t) == 0x43380000) ? m : 0;
+    uint32_t r3, adr, lo, hi;
     asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
     asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(adr) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8), "r"(tab));   // (a & b) | c
     asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(adr));
+#ifdef BLTC_X_LOPMERGE
+    uint32_t rx, hi2;
     asm("shf.l.wrap.b32 %0, %1, %1, %2;" : "=r"(rx) : "r"(m), "n"(20 - BLTC_EXP_LOG2T));
     asm("lop3.b32 %0, %1, %2, %3, 0xE2;" : "=r"(hi2) : "r"(rx), "n"(0x7FF00000), "r"(hi));              // (a & b) | (c & ~b)
+#else
+    const uint32_t hi2 = hi + ((uint32_t)m << (20 - BLTC_EXP_LOG2T));       // exponent n + 1023 merged by one shift-add
+#endif
     const double tj = __hiloint2double((int)hi2, (int)lo);   // 2^n * 2^(j/T)
-    double p = fma(rho, BLTC_EXP_C3, mr.c2);
-    p = fma(p, rho, BLTC_EXP_C1);
-    const double s = tj * rho;
-    return fma(s, p, tj);                               // tj (1 + rho p(rho))
+    double p = fma(rho, ec.c3, mr.c2);
+    p = fma(p, rho, ec.c1);
+    const double q = p * rho;
+    return fma(tj, q, tj);                              // tj (1 + rho p(rho)); two distinct register operands
 }
 
 // host side: c = -k T / ln2, rounded once from extended precision

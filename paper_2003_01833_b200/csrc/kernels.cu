@@ -20,13 +20,31 @@
 
 #include "fp64_math.cuh"
 
+// experimental switches (tuning only)
+#ifndef BLTC_X_UNROLL
+#define BLTC_X_UNROLL 2
+#endif
+#ifndef BLTC_X_MINCTAS
+#define BLTC_X_MINCTAS 2
+#endif
+#ifdef BLTC_X_NOZERO
+#define BLTC_X_ZS false
+#else
+#define BLTC_X_ZS true
+#endif
+#ifndef BLTC_X_FUNROLL
+#define BLTC_X_FUNROLL 2
+#endif
+
 namespace bltc {
 namespace {
 
+constexpr int kXUnroll = BLTC_X_UNROLL, kXFUnroll = BLTC_X_FUNROLL;
+
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
-// {0.375, BLTC_EXP_C2}: constants the pair kernels keep in registers (see fp64_math.cuh, MathRegs)
-__device__ double kMathOpaque[2] = {0.375, BLTC_EXP_C2};
+// {0.375, BLTC_EXP_C2, kExpMagic}: constants the pair kernels keep in registers (see fp64_math.cuh, MathRegs)
+__device__ double kMathOpaque[3] = {0.375, BLTC_EXP_C2, kExpMagic};
 
 // ------------------------------------------------------------------------------------ a1 / pack
 __global__ void gather_kernel(const double* __restrict__ f, int64_t stride, int o0, int ot,
@@ -217,21 +235,67 @@ __device__ __forceinline__ void reduce_and_store(TargetRegs<R, OT>& T, const Wor
 }
 
 // ------------------------------------------------------------------------------------ a4 / a6
-template <int R, int OT, bool SUB>
-__global__ void __launch_bounds__(kThreads, 2)
+// Shared-memory tile of sources: one record {x, y, z, w, f[OT]} per source, padded to a multiple of
+// 16 bytes, so one source is 3-4 LDS.128 at immediate offsets from one running pointer.  The S
+// source-split ways of a tile take contiguous chunks of it (broadcast reads: no bank conflicts).
+template <int OT> struct SrcRec { static constexpr int kDoubles = OT <= 2 ? 6 : 8; };
+
+// ZS (zero-safe): the tile may hold a source that coincides with a target -> the singular term is
+// skipped by an integer select on the rsqrt seed (reading R3).  The host flags the
+// ranges for which that can happen (bounding boxes intersect); all other tiles run the ZS = false loop.
+template <int R, int OT, bool SUB, bool GUARD, bool ZS>
+__device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __restrict__ tile, int j0, int j1,
+                                          const KPar& kp, uint32_t tab, const MathRegs& mr) {
+    constexpr int RD = SrcRec<OT>::kDoubles;
+    const ExpConst ec{kp.c1, kp.c3};
+#pragma unroll kXUnroll
+    for (int j = j0; j < j1; ++j) {
+        const double* s = tile + j * RD;
+        const double2 sxy = *reinterpret_cast<const double2*>(s);
+        const double2 szw = *reinterpret_cast<const double2*>(s + 2);
+        double sf[OT];
+#pragma unroll
+        for (int o = 0; o < OT; o += 2) {
+            if (o + 1 < OT) {
+                const double2 v = *reinterpret_cast<const double2*>(s + 4 + o);
+                sf[o] = v.x; sf[o + 1] = v.y;
+            } else {
+                sf[o] = s[4 + o];
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double dx = T.x[r] - sxy.x, dy = T.y[r] - sxy.y, dz = T.z[r] - szw.x;
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double rinv, rr;
+            rsqrt_sqrt<ZS>(r2, rinv, rr, mr);              // ZS and r2 == 0: rinv = 0, the term vanishes
+            const double gw = rinv * szw.y;
+#pragma unroll
+            for (int o = 0; o < OT; ++o) {
+                const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
+                const double g = ex * gw;
+                const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
+                T.acc[r][o] = fma(g, df, T.acc[r][o]);
+            }
+        }
+    }
+}
+
+template <int R, int OT, bool SUB, bool GUARD>
+__global__ void __launch_bounds__(kThreads, BLTC_X_MINCTAS)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
             const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
             double* __restrict__ partial, int64_t partial_len) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    static_assert(sizeof(double4) * kSrcTile >= sizeof(double) * R * OT * 8 * 32, "reduction scratch");
+    constexpr int RD = SrcRec<OT>::kDoubles;
+    static_assert(RD * kSrcTile >= R * OT * 8 * 32, "reduction scratch fits in the tile");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
-    double4* s_rec = reinterpret_cast<double4*>(smem_raw + 2 * kExpTableBytes);
-    double* s_f = reinterpret_cast<double*>(s_rec + kSrcTile);
+    double* s_tile = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
-    const int G = 1 << it.gshift, S = 8 >> it.gshift;
+    const int G = 1 << it.gshift, sshift = 3 - it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
     TargetRegs<R, OT> T;
     load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
@@ -240,48 +304,33 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
     int at = q < it.list_end ? ranges[q].begin : 0;
     while (q < it.list_end) {
         __syncthreads();                                   // previous tile consumed (and table ready)
-        int fill = 0;
+        int fill = 0, flags = 0;
         while (fill < kSrcTile && q < it.list_end) {
-            const int end = ranges[q].end;
-            const int n = min(kSrcTile - fill, end - at);
+            const Range rg = ranges[q];
+            const int n = min(kSrcTile - fill, rg.end - at);
+            flags |= rg.flags;
             for (int i = tid; i < n; i += kThreads) {
-                s_rec[fill + i] = src_rec[at + i];
+                const double4 v = src_rec[at + i];
+                double* d = s_tile + (fill + i) * RD;
+                *reinterpret_cast<double2*>(d) = make_double2(v.x, v.y);
+                *reinterpret_cast<double2*>(d + 2) = make_double2(v.z, v.w);
 #pragma unroll
-                for (int o = 0; o < OT; ++o) s_f[(fill + i) * OT + o] = fsrc[(size_t)(at + i) * OT + o];
+                for (int o = 0; o < OT; ++o) d[4 + o] = fsrc[(size_t)(at + i) * OT + o];
             }
             fill += n; at += n;
-            if (at == end) { ++q; if (q < it.list_end) at = ranges[q].begin; }
+            if (at == rg.end) { ++q; if (q < it.list_end) at = ranges[q].begin; }
         }
         __syncthreads();
-#pragma unroll 2
-        for (int j = split; j < fill; j += S) {
-            const double4 s = s_rec[j];
-            double sf[OT];
-#pragma unroll
-            for (int o = 0; o < OT; ++o) sf[o] = s_f[j * OT + o];
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const double dx = T.x[r] - s.x, dy = T.y[r] - s.y, dz = T.z[r] - s.z;
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                double rinv, rr;
-                rsqrt_sqrt<true>(r2, rinv, rr, mr);        // r2 == 0: rinv = 0, the term vanishes
-                const double gw = rinv * s.w;
-#pragma unroll
-                for (int o = 0; o < OT; ++o) {
-                    const double ex = exp_neg_kr(rr, kp.c[o], tab, mr);
-                    const double g = ex * gw;
-                    const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
-                    T.acc[r][o] = fma(g, df, T.acc[r][o]);
-                }
-            }
-        }
+        const int j0 = (fill * split) >> sshift, j1 = (fill * (split + 1)) >> sshift;
+        if (flags & kRangeMayCoincide) near_tile<R, OT, SUB, GUARD, true>(T, s_tile, j0, j1, kp, tab, mr);
+        else near_tile<R, OT, SUB, GUARD, false>(T, s_tile, j0, j1, kp, tab, mr);
     }
-    reduce_and_store<R, OT>(T, it, warp, lane, split, S, reinterpret_cast<double*>(s_rec), partial, partial_len);
+    reduce_and_store<R, OT>(T, it, warp, lane, split, 8 >> it.gshift, s_tile, partial, partial_len);
 }
 
 // ------------------------------------------------------------------------------------ a3
-template <int R, int OT, bool SUB>
-__global__ void __launch_bounds__(kThreads, 2)
+template <int R, int OT, bool SUB, bool GUARD>
+__global__ void __launch_bounds__(kThreads, BLTC_X_MINCTAS)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
            const double* __restrict__ fhat, int n1, const double4* __restrict__ tgt_rec,
@@ -295,6 +344,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     double* s_fh = s_w + kProxyTile;
     double* s_nodes = s_fh + kProxyTile * OT;            // [3][21]
     const MathRegs mr = math_regs_init(kMathOpaque);
+    const ExpConst ec{kp.c1, kp.c3};
     const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, S = 8 >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
@@ -329,7 +379,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
                     dxy2[r] = fma(dy, dy, dx * dx);
                 }
                 const int pbase = row * n1;
-#pragma unroll 2
+#pragma unroll kXFUnroll
                 for (int k3 = 0; k3 < n1; ++k3) {
                     const double sz = s_nodes[2 * n1 + k3];
                     const double wv = SUB ? s_w[pbase + k3] : 0.0;
@@ -344,7 +394,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
                         rsqrt_sqrt<false>(r2, rinv, rr, mr);   // MAC keeps targets off the grid (theta < 1)
 #pragma unroll
                         for (int o = 0; o < OT; ++o) {
-                            const double ex = exp_neg_kr(rr, kp.c[o], tab, mr);
+                            const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
                             const double g = ex * rinv;
                             // fhat_k - f_i what_k: interpolated charges of (f_j - f_i) w_j (reading R11)
                             const double qk = SUB ? fma(-T.f[r][o], wv, fv[o]) : fv[o];
@@ -402,7 +452,7 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
-size_t near_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + kSrcTile * (sizeof(double4) + sizeof(double) * ot); }
+size_t near_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + (size_t)kSrcTile * sizeof(double) * (ot <= 2 ? 6 : 8); }
 size_t far_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + sizeof(double) * (kProxyTile * (1 + (size_t)ot) + 3 * 21); }
 
 template <typename K>
@@ -421,6 +471,8 @@ KPar make_kpar(const double* k, int ot) {
         kp.nk[o] = -kk;
         kp.c[o] = exp_scale_of_k(kk);
     }
+    kp.c1 = BLTC_EXP_C1;
+    kp.c3 = BLTC_EXP_C3;
     return kp;
 }
 
@@ -461,69 +513,50 @@ cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const in
     return cudaGetLastError();
 }
 
-cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
+// kernel<R, OT, SUB, GUARD> dispatch on (ot, subtract, guard): R = 2 for ot <= 2, else 1
+template <template <int, int, bool, bool> class K, typename... Args>
+cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int grid, cudaStream_t st, Args... args) {
+#define BLTC_GO(RV, OTV, SV, GV)                                                                        \
+    {                                                                                                   \
+        auto kern = K<RV, OTV, SV, GV>::get();                                                          \
+        cudaError_t e = set_smem(kern, smem);                                                           \
+        if (e != cudaSuccess) return e;                                                                 \
+        kern<<<grid, kThreads, smem, st>>>(args...);                                                    \
+        return cudaGetLastError();                                                                      \
+    }
+#define BLTC_SG(RV, OTV)                                                                                \
+    if (subtract) { if (guard) BLTC_GO(RV, OTV, true, true) else BLTC_GO(RV, OTV, true, false) }        \
+    else { if (guard) BLTC_GO(RV, OTV, false, true) else BLTC_GO(RV, OTV, false, false) }
+    switch (ot) {
+        case 1: BLTC_SG(2, 1)
+        case 2: BLTC_SG(2, 2)
+        case 3: BLTC_SG(1, 3)
+        case 4: BLTC_SG(1, 4)
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_SG
+#undef BLTC_GO
+}
+
+template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD>; } };
+
+cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
-    const int n1 = degree + 1;
-    cudaError_t e = cudaSuccess;
-#define BLTC_FAR(RV, OTV)                                                                               \
-    {                                                                                                   \
-        const size_t smem = far_smem_bytes(OTV);                                                        \
-        if (subtract) {                                                                                 \
-            e = set_smem(far_kernel<RV, OTV, true>, smem);                                              \
-            if (e != cudaSuccess) return e;                                                             \
-            far_kernel<RV, OTV, true><<<nitems, kThreads, smem, st>>>(items, far_slots, slot_nodes,     \
-                what, fhat, n1, tgt_rec, ftgt, kp, partial, partial_len);                               \
-        } else {                                                                                        \
-            e = set_smem(far_kernel<RV, OTV, false>, smem);                                             \
-            if (e != cudaSuccess) return e;                                                             \
-            far_kernel<RV, OTV, false><<<nitems, kThreads, smem, st>>>(items, far_slots, slot_nodes,    \
-                what, fhat, n1, tgt_rec, ftgt, kp, partial, partial_len);                               \
-        }                                                                                               \
-    }
-    switch (ot) {
-        case 1: BLTC_FAR(2, 1) break;
-        case 2: BLTC_FAR(2, 2) break;
-        case 3: BLTC_FAR(1, 3) break;
-        case 4: BLTC_FAR(1, 4) break;
-        default: return cudaErrorInvalidValue;
-    }
-#undef BLTC_FAR
-    return cudaGetLastError();
+    return dispatch_pair<FarK>(ot, subtract, guard, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
+                               what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
 }
 
-cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
+cudaError_t launch_near(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
-    cudaError_t e = cudaSuccess;
-#define BLTC_NEAR(RV, OTV)                                                                              \
-    {                                                                                                   \
-        const size_t smem = near_smem_bytes(OTV);                                                       \
-        if (subtract) {                                                                                 \
-            e = set_smem(near_kernel<RV, OTV, true>, smem);                                             \
-            if (e != cudaSuccess) return e;                                                             \
-            near_kernel<RV, OTV, true><<<nitems, kThreads, smem, st>>>(items, ranges, src_rec, fsrc,    \
-                tgt_rec, ftgt, kp, partial, partial_len);                                               \
-        } else {                                                                                        \
-            e = set_smem(near_kernel<RV, OTV, false>, smem);                                            \
-            if (e != cudaSuccess) return e;                                                             \
-            near_kernel<RV, OTV, false><<<nitems, kThreads, smem, st>>>(items, ranges, src_rec, fsrc,   \
-                tgt_rec, ftgt, kp, partial, partial_len);                                               \
-        }                                                                                               \
-    }
-    switch (ot) {
-        case 1: BLTC_NEAR(2, 1) break;
-        case 2: BLTC_NEAR(2, 2) break;
-        case 3: BLTC_NEAR(1, 3) break;
-        case 4: BLTC_NEAR(1, 4) break;
-        default: return cudaErrorInvalidValue;
-    }
-#undef BLTC_NEAR
-    return cudaGetLastError();
+    return dispatch_pair<NearK>(ot, subtract, guard, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc,
+                                tgt_rec, ftgt, kp, partial, partial_len);
 }
 
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,

@@ -16,8 +16,10 @@ constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile
 inline int targets_per_thread(int ot) { return ot <= 2 ? 2 : 1; }
 
 // per-orbital constants of the tile (kernel parameter -> constant bank):
-//   nk = -k_o;  c = -k_o T/ln2 (scaled exponent argument of fp64_math.cuh's exp)
-struct KPar { double nk[kMaxOT]; double c[kMaxOT]; };
+//   nk = -k_o;  c = -k_o T/ln2 (scaled exponent argument of fp64_math.cuh's exp);  c1, c3: polynomial
+//   coefficients of that exp (kept in uniform registers)
+// guard (launch_far / launch_near): false only if k r < 700 for every pair of the launch (no exp underflow)
+struct KPar { double nk[kMaxOT]; double c[kMaxOT]; double c1, c3; };
 KPar make_kpar(const double* k, int ot);   // k: ot values (host)
 
 // a1: f[o0+o][perm[i]] -> dst[i][ot] (tree order, orbital-interleaved)
@@ -34,13 +36,13 @@ cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const in
                           const double* fsrc, double* out, cudaStream_t st);
 
 // a3: far field
-cudaError_t launch_far(int ot, bool subtract, const WorkItem* items, int nitems, const int32_t* far_slots,
+cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st);
 
 // a4 / a6: near field and brute-force direct sum (same kernel, different work items)
-cudaError_t launch_near(int ot, bool subtract, const WorkItem* items, int nitems, const Range* ranges,
+cudaError_t launch_near(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st);

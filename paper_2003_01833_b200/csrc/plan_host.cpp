@@ -176,6 +176,16 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         build_tree(p.tgt, t, t + N, t + 2 * N, N, batch_size);
         bt = &p.tgt;
     }
+    {   // bound of |target - source|: farthest corners of the two root boxes
+        const Cluster& A = p.src.cl[0];
+        const Cluster& B = bt->cl[0];
+        double d2 = 0.0;
+        for (int d = 0; d < 3; ++d) {
+            const double e = std::max(A.hi[d], B.hi[d]) - std::min(A.lo[d], B.lo[d]);
+            d2 += e * e;
+        }
+        p.max_dist = std::sqrt(d2);
+    }
     const int nb = (int)bt->leaves.size();
     p.b_begin.resize(nb); p.b_end.resize(nb); p.b_lo.resize(3 * (size_t)nb); p.b_hi.resize(3 * (size_t)nb);
     for (int b = 0; b < nb; ++b) {
@@ -232,12 +242,17 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         std::vector<Range>& r = merged[b];
         for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
             const Cluster& C = p.src.cl[p.near_idx[q]];
-            r.push_back(Range{(int32_t)C.begin, (int32_t)C.end});
+            // can a source of C coincide with a target of the batch?  Only if the (closed, minimal)
+            // bounding boxes intersect; otherwise the kernel skips the r == 0 test (reading R3).
+            bool touch = true;
+            for (int d = 0; d < 3; ++d)
+                touch = touch && C.lo[d] <= p.b_hi[3 * b + d] && p.b_lo[3 * b + d] <= C.hi[d];
+            r.push_back(Range{(int32_t)C.begin, (int32_t)C.end, touch ? kRangeMayCoincide : 0});
         }
         std::sort(r.begin(), r.end(), [](const Range& a, const Range& c) { return a.begin < c.begin; });
         size_t o = 0;
         for (size_t i = 0; i < r.size(); ++i) {
-            if (o > 0 && r[o - 1].end == r[i].begin) r[o - 1].end = r[i].end;
+            if (o > 0 && r[o - 1].end == r[i].begin && r[o - 1].flags == r[i].flags) r[o - 1].end = r[i].end;
             else r[o++] = r[i];
         }
         r.resize(o);
@@ -266,7 +281,7 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
                 int32_t at = g.begin;
                 while (at < g.end) {
                     const int32_t take = (int32_t)std::min<int64_t>(room, g.end - at);
-                    p.near_ranges.push_back(Range{at, at + take});
+                    p.near_ranges.push_back(Range{at, at + take, g.flags});
                     at += take; room -= take;
                     if (room == 0) {
                         nseg_slices.emplace_back(seg_start, (int32_t)p.near_ranges.size());

@@ -35,7 +35,10 @@ struct WorkItem {
     int64_t partial_off;             // where this (batch, segment) slice starts in the partial buffer
 };
 
-struct Range { int32_t begin, end; };   // source range in tree order
+// source range in tree order; flags & kRangeMayCoincide: a source of the range may coincide with a
+// target of the batch (their bounding boxes intersect), so the kernel must test r == 0 (reading R3)
+struct Range { int32_t begin, end, flags; };
+constexpr int32_t kRangeMayCoincide = 1;
 
 struct HostPlan {
     // parameters
@@ -71,6 +74,7 @@ struct HostPlan {
     int64_t partial_len = 0;                   // doubles per orbital
     std::vector<WorkItem> far_items[2], near_items[2];   // [0]: R = 1 (32 targets/group), [1]: R = 2
 
+    double max_dist = 0;                       // upper bound of |target - source| over all pairs (root boxes)
     double build_ms = 0;
 };
 

@@ -3,9 +3,9 @@
 
   python -m paper_2003_01833_b200.sass_count [--md]
 
-For every near_kernel<R,OT,SUB> / far_kernel<R,OT,SUB> instantiation the innermost loop that contains
-MUFU.RSQ64H (one per (target, source-or-proxy) pair) is located through its backward branch and its
-opcodes are counted.  "pair" = one target against one source / proxy point, ALL OT orbitals of the tile;
+For every near_kernel<R,OT,SUB,GUARD> / far_kernel<R,OT,SUB,GUARD> instantiation the innermost loops that
+contain MUFU.RSQ64H (one per (target, source-or-proxy) pair) are located through their backward branches
+and their opcodes are counted (near: one loop per ZS variant, ZS = the r == 0 test is compiled in).  "pair" = one target against one source / proxy point, ALL OT orbitals of the tile;
 flops = 2 DFMA + DMUL + DADD.  bench.py's FLOPS_PER_PAIR table holds the SUB = 1 rows.
 Needs cuobjdump (CUDA toolkit); no GPU.
 """
@@ -33,47 +33,48 @@ def kernels(lib):
     return out
 
 
-def inner_loop(ins):
+def pair_loops(ins):
+    """Innermost backward-branch loops that contain MUFU.RSQ64H (one per (target, source) pair)."""
     mufu = [a for a, t in ins if "MUFU.RSQ64H" in t]
-    best = None
+    loops = []
     for a, t in ins:
         m = re.search(r"BRA(?:\.U)?\s+(?:!?U?P\d+,\s*)?0x([0-9a-f]+)", t)
         if not m:
             continue
         tgt = int(m.group(1), 16)
         if tgt < a and any(tgt <= x <= a for x in mufu):
-            if best is None or (a - tgt) < (best[1] - best[0]):
-                best = (tgt, a)
-    return best
+            loops.append((tgt, a))
+    inner = [l for l in loops if not any(o != l and l[0] <= o[0] and o[1] <= l[1] for o in loops)]
+    return inner
 
 
 def count(lib=None):
     lib = lib or _build.build()
     rows = []
     for name, ins in kernels(lib).items():
-        m = re.search(r"(near_kernel|far_kernel)ILi(\d)ELi(\d)ELb([01])E", name)
+        m = re.search(r"(near_kernel|far_kernel)ILi(\d)ELi(\d)ELb([01])ELb([01])E", name)
         if not m:
             continue
-        lp = inner_loop(ins)
-        if not lp:
-            continue
-        body = [t for a, t in ins if lp[0] <= a <= lp[1]]
-        ops = [re.sub(r"^@!?U?P\d+\s+", "", t).split()[0].split(".")[0] for t in body]
-        pairs = sum("MUFU.RSQ64H" in t for t in body)
-        c = {k: ops.count(k) / pairs for k in ("DFMA", "DMUL", "DADD")}
-        fp64 = c["DFMA"] + c["DMUL"] + c["DADD"]
-        fma_pipe = sum(o in ("IMAD", "FFMA", "FMUL", "FADD") for o in ops) / pairs
-        rows.append(dict(kernel=m.group(1), R=int(m.group(2)), OT=int(m.group(3)), SUB=int(m.group(4)),
-                         pairs=pairs, **c, fp64=fp64, other=len(ops) / pairs - fp64, fma_pipe=fma_pipe,
-                         flops=2 * c["DFMA"] + c["DMUL"] + c["DADD"]))
-    rows.sort(key=lambda r: (r["kernel"], r["R"], r["OT"], r["SUB"]))
+        for lp in pair_loops(ins):
+            body = [t for a, t in ins if lp[0] <= a <= lp[1]]
+            ops = [re.sub(r"^@!?U?P\d+\s+", "", t).split()[0].split(".")[0] for t in body]
+            pairs = sum("MUFU.RSQ64H" in t for t in body)
+            zs = int(any("ISETP" in t and "0x7ff00000" in t for t in body))
+            c = {k: ops.count(k) / pairs for k in ("DFMA", "DMUL", "DADD")}
+            fp64 = c["DFMA"] + c["DMUL"] + c["DADD"]
+            fma_pipe = sum(o in ("IMAD", "FFMA", "FMUL", "FADD") for o in ops) / pairs
+            rows.append(dict(kernel=m.group(1), R=int(m.group(2)), OT=int(m.group(3)), SUB=int(m.group(4)),
+                             GUARD=int(m.group(5)), ZS=zs, pairs=pairs, **c, fp64=fp64,
+                             other=len(ops) / pairs - fp64, fma_pipe=fma_pipe,
+                             flops=2 * c["DFMA"] + c["DMUL"] + c["DADD"]))
+    rows.sort(key=lambda r: (r["kernel"], r["R"], r["OT"], r["SUB"], r["GUARD"], r["ZS"]))
     return rows
 
 
 def main():
     rows = count()
-    hdr = ["kernel", "R", "OT", "SUB", "pairs", "DFMA", "DMUL", "DADD", "fp64", "other", "fma_pipe", "flops"]
-    names = ["kernel", "R", "OT", "SUB", "pairs/iter", "DFMA/pair", "DMUL/pair", "DADD/pair", "FP64 instr/pair",
+    hdr = ["kernel", "R", "OT", "SUB", "GUARD", "ZS", "pairs", "DFMA", "DMUL", "DADD", "fp64", "other", "fma_pipe", "flops"]
+    names = ["kernel", "R", "OT", "SUB", "GUARD", "ZS", "pairs/iter", "DFMA/pair", "DMUL/pair", "DADD/pair", "FP64 instr/pair",
              "other instr/pair", "of which FMA-pipe", "flops/pair"]
     if "--md" in sys.argv:
         print("| " + " | ".join(names) + " |")

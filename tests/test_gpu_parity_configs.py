@@ -1,0 +1,126 @@
+"""GPU parity at BASELINE.json's full sizes (configs 2, 3, 4), in the launch configuration the library
+uses for them: sampled target batches against the CPU BLTC oracle (batches are independent, so the
+oracle's values for those targets are exact, not approximate), sampled targets against the CPU direct
+sum, and the BLTC-vs-direct error of the method.  Tolerances as in test_gpu_parity.py.
+
+The oracle evaluates a subset of the orbitals (one per register-tile group of the library at least):
+orbitals are independent of each other in the method, the subset only bounds the CPU time.
+"""
+import numpy as np
+import pytest
+
+from paper_2003_01833_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL_DIRECT = 1e-13
+TOL_BLTC = 1e-12
+
+
+def rel2(a, b):
+    a = np.atleast_2d(a); b = np.atleast_2d(b)
+    return max(float(np.linalg.norm(a[o] - b[o]) / np.linalg.norm(b[o])) for o in range(a.shape[0]))
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2003_01833_b200 import binding as B
+    B.lib()
+    return torch, B
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_bltc(gpu, c, subtract):
+    torch, B = gpu
+    plan = B.bltc_create(None, dev(torch, c.coords()), dev(torch, c.w), c.N, c.theta, c.degree,
+                         c.batch_size, c.leaf_size)
+    out = torch.empty((c.n_orb, c.N), dtype=torch.float64, device="cuda")
+    B.bltc_convolve(plan, c.k, dev(torch, c.f), c.n_orb, out, subtract)
+    torch.cuda.synchronize()
+    st = B.bltc_get_stats(plan)
+    B.bltc_destroy(plan)
+    return out.cpu().numpy(), st
+
+
+def run_direct(gpu, c, idx, subtract):
+    torch, B = gpu
+    X = c.coords()
+    out = torch.empty((c.n_orb, len(idx)), dtype=torch.float64, device="cuda")
+    B.direct_convolve(dev(torch, X[:, idx]), dev(torch, c.f[:, idx]) if subtract else None, len(idx),
+                      dev(torch, X), dev(torch, c.w), dev(torch, c.f), c.N, c.k, c.n_orb, out, subtract)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def check_full_size(gpu, oracle_mod, c, batches, orbitals, subtract, n_direct=600, n_cpu_direct=60,
+                    tol_method=None):
+    got, st = run_bltc(gpu, c, subtract)
+    assert np.all(np.isfinite(got))
+    P = (c.x, c.y, c.z)
+    op = oracle_mod.OraclePlan(P, c.theta, c.degree, c.leaf_size, c.batch_size)
+    assert (st["n_clusters"], st["n_batches"], st["far_evals"], st["near_evals"]) == \
+           (op.n_clusters, op.n_batches, op.far_evals, op.near_evals)
+    batches = [b % op.n_batches for b in batches]
+    ref = op.evaluate(c.w, c.f[orbitals], c.k[orbitals], batches=batches, subtract=subtract)
+    m = np.isfinite(ref[0])
+    assert m.sum() >= 32
+    e_tc = rel2(got[orbitals][:, m], ref[:, m])
+    # GPU direct on sampled targets (all orbitals); CPU direct on a few of them pins the GPU direct
+    idx = I.sample_targets(c.N, n_direct, seed=c.N % 97)
+    gd = run_direct(gpu, c, idx, subtract)
+    sub = idx[:n_cpu_direct]
+    dref = oracle_mod.direct((c.x[sub], c.y[sub], c.z[sub]), P, c.w, c.f[orbitals], c.k[orbitals],
+                             f_tgt=c.f[orbitals][:, sub], subtract=subtract)
+    e_ds = rel2(gd[orbitals][:, :n_cpu_direct], dref)
+    e_method = rel2(got[:, idx], gd)
+    print(f"{c.name} theta={c.theta} n={c.degree}: GPU BLTC vs CPU BLTC {e_tc:.2e}, GPU direct vs CPU direct "
+          f"{e_ds:.2e}, BLTC vs direct (all {c.n_orb} orbitals, {len(idx)} targets) {e_method:.2e}")
+    assert e_tc <= TOL_BLTC
+    assert e_ds <= TOL_DIRECT
+    if tol_method is not None:
+        assert e_method <= tol_method
+    return e_method
+
+
+@pytest.mark.parametrize("theta,degree,tol", [(0.8, 6, 1e-4), (0.6, 8, 1e-6)])
+def test_config2_co_like(gpu, oracle_mod, theta, degree, tol):
+    # BASELINE.json configs[2]: theta in {0.6, 0.8}, degree in {6, 8}; 7 orbitals = register tiles 4 + 3
+    c = I.config2(theta=theta, degree=degree)
+    check_full_size(gpu, oracle_mod, c, batches=[3, 611], orbitals=[0, 3, 4, 6], subtract=True, tol_method=tol)
+
+
+def test_config2_error_decreases_with_degree_and_smaller_theta(gpu):
+    # PAPER.md:472 Fig. 10: the treecode error falls as n grows and theta shrinks (GPU path only, vs GPU direct)
+    errs = {}
+    for theta, degree in [(0.8, 6), (0.8, 8), (0.6, 8)]:
+        c = I.config2(theta=theta, degree=degree)
+        c.f = np.ascontiguousarray(c.f[[0, 6]]); c.k = c.k[[0, 6]]
+        got, _ = run_bltc(gpu, c, True)
+        idx = I.sample_targets(c.N, 400, seed=3)
+        errs[(theta, degree)] = rel2(got[:, idx], run_direct(gpu, c, idx, True))
+    print("config2 BLTC-vs-direct:", errs)
+    assert errs[(0.8, 8)] < errs[(0.8, 6)] and errs[(0.6, 8)] < errs[(0.8, 8)]
+
+
+def test_config3_c6h6_like(gpu, oracle_mod):
+    # BASELINE.json configs[3]: 3.46 M points, 21 orbitals (register tiles 4,4,4,3,3,3), theta 0.7, degree 8
+    c = I.config3()
+    check_full_size(gpu, oracle_mod, c, batches=[17, 4242], orbitals=[0, 7, 13, 20], subtract=True,
+                    n_direct=300, n_cpu_direct=24, tol_method=1e-6)
+
+
+@pytest.mark.parametrize("k,theta,degree", [(0.5, 0.7, 8), (5.0, 0.9, 4), (1.0, 0.5, 10)])
+def test_config4_random_cube(gpu, oracle_mod, k, theta, degree):
+    # BASELINE.json configs[4] at N = 1e6 (subtraction off: the points are not a quadrature)
+    c = I.config4(N=1_000_000, k=k, theta=theta, degree=degree)
+    e = check_full_size(gpu, oracle_mod, c, batches=[1, 500], orbitals=[0], subtract=False,
+                        n_direct=2000, n_cpu_direct=100)
+    if (theta, degree) == (0.7, 8):
+        assert e <= 1e-6
+    if (theta, degree) == (0.5, 10):
+        assert e <= 1e-9

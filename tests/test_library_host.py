@@ -87,3 +87,21 @@ def test_host_plan_separate_targets(oracle_mod):
     for key in e:
         np.testing.assert_array_equal(e[key], oe[key], err_msg=key)
     assert B.bltc_get_stats(p)["shared_batches"] == 0
+
+
+def test_bench_flops_table_matches_the_built_sass():
+    """bench.py's FLOPS_PER_PAIR (the roofline numerator) is the FP64 instruction mix actually in the
+    pair kernels' inner loops of the built library, re-counted here from cuobjdump -sass."""
+    import shutil
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump not on PATH")
+    import bench
+    from paper_2003_01833_b200 import sass_count
+    rows = [r for r in sass_count.count() if r["SUB"] == 1]
+    seen = set()
+    for r in rows:                      # every GUARD / ZS variant executes the same FP64 mix per pair
+        key = ("near" if r["kernel"] == "near_kernel" else "far", r["OT"])
+        assert bench.FLOPS_PER_PAIR[key] == pytest.approx(r["flops"], abs=1e-9), (key, r)
+        assert r["R"] == (2 if r["OT"] <= 2 else 1)
+        seen.add(key)
+    assert seen == set(bench.FLOPS_PER_PAIR)
