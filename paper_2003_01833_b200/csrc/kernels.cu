@@ -329,20 +329,32 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 }
 
 // ------------------------------------------------------------------------------------ a3
-template <int R, int OT, bool SUB, bool GUARD>
+// Shared-memory tile of proxy points: one record {what_k, fhat_k[OT]} per point (padded to 16 bytes),
+// k3 fastest, so a (k1, k2) row of the tensor grid is n1 consecutive records.  N1 > 0: the grid size
+// degree + 1 is a compile-time constant and the k3 loop is fully unrolled (no remainder iteration, the
+// next row's dx^2 + dy^2 overlaps the tail of the current one); N1 = 0: any degree.
+template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 : (OT <= 3 ? 4 : 6); };
+
+template <int R, int OT, bool SUB, bool GUARD, int N1>
 __global__ void __launch_bounds__(kThreads, BLTC_X_MINCTAS)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
-           const double* __restrict__ fhat, int n1, const double4* __restrict__ tgt_rec,
+           const double* __restrict__ fhat, int n1_arg, const double4* __restrict__ tgt_rec,
            const double* __restrict__ ftgt, const KPar kp, double* __restrict__ partial,
            int64_t partial_len) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    static_assert(kProxyTile >= R * 8 * 32, "reduction scratch fits in s_fh");
+    constexpr int PD = ProxyRec<OT>::kDoubles;
+    static_assert(kProxyTile * PD >= R * OT * 8 * 32, "reduction scratch fits in the tile");
+#ifdef BLTC_X_F9UNROLL
+    constexpr int kU = N1 ? BLTC_X_F9UNROLL : kXFUnroll;
+#else
+    constexpr int kU = N1 ? N1 : kXFUnroll;
+#endif
+    const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
-    double* s_w = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
-    double* s_fh = s_w + kProxyTile;
-    double* s_nodes = s_fh + kProxyTile * OT;            // [3][21]
+    double* s_pts = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
+    double* s_nodes = s_pts + kProxyTile * PD;           // [3][21]
     const MathRegs mr = math_regs_init(kMathOpaque);
     const ExpConst ec{kp.c1, kp.c3};
     const WorkItem it = items[blockIdx.x];
@@ -364,28 +376,45 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
                 for (int i = tid; i < 3 * n1; i += kThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
             const size_t base = (size_t)slot * P + (size_t)k1a * plane;
             for (int i = tid; i < npts; i += kThreads) {
-                if (SUB) s_w[i] = what[base + i];
+                double* d = s_pts + i * PD;
+                d[0] = SUB ? what[base + i] : 0.0;
 #pragma unroll
-                for (int o = 0; o < OT; ++o) s_fh[i * OT + o] = fhat[(base + i) * OT + o];
+                for (int o = 0; o < OT; ++o) d[1 + o] = fhat[(base + i) * OT + o];
             }
             __syncthreads();
             const int rows = (k1b - k1a) * n1;
             for (int row = split; row < rows; row += S) {
-                const int k1 = k1a + row / n1, k2 = row % n1;
+                const int kq = row / n1;
+                const int k1 = k1a + kq, k2 = row - kq * n1;
                 double dxy2[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const double dx = T.x[r] - s_nodes[k1], dy = T.y[r] - s_nodes[n1 + k2];
                     dxy2[r] = fma(dy, dy, dx * dx);
                 }
-                const int pbase = row * n1;
-#pragma unroll kXFUnroll
+                const double* pr = s_pts + row * n1 * PD;
+                const double* pz = s_nodes + 2 * n1;
+#pragma unroll kU
                 for (int k3 = 0; k3 < n1; ++k3) {
-                    const double sz = s_nodes[2 * n1 + k3];
-                    const double wv = SUB ? s_w[pbase + k3] : 0.0;
-                    double fv[OT];
+                    const double sz = pz[k3];
+                    const double* rec = pr + k3 * PD;
+                    double wv, fv[OT];
+                    if (OT == 1) {
+                        const double2 v = *reinterpret_cast<const double2*>(rec);
+                        wv = v.x; fv[0] = v.y;
+                    } else {
+                        const double2 v = *reinterpret_cast<const double2*>(rec);
+                        wv = v.x; fv[0] = v.y;
 #pragma unroll
-                    for (int o = 0; o < OT; ++o) fv[o] = s_fh[(pbase + k3) * OT + o];
+                        for (int o = 1; o < OT; o += 2) {
+                            if (o + 1 < OT) {
+                                const double2 u = *reinterpret_cast<const double2*>(rec + 1 + o);
+                                fv[o] = u.x; fv[o + 1] = u.y;
+                            } else {
+                                fv[o] = rec[1 + o];
+                            }
+                        }
+                    }
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const double dz = T.z[r] - sz;
@@ -405,7 +434,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
             }
         }
     }
-    reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_fh, partial, partial_len);
+    reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_pts, partial, partial_len);
 }
 
 // ------------------------------------------------------------------------------------ a5
@@ -453,7 +482,7 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
 }
 
 size_t near_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + (size_t)kSrcTile * sizeof(double) * (ot <= 2 ? 6 : 8); }
-size_t far_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + sizeof(double) * (kProxyTile * (1 + (size_t)ot) + 3 * 21); }
+size_t far_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + sizeof(double) * ((size_t)kProxyTile * (ot == 1 ? 2 : (ot <= 3 ? 4 : 6)) + 3 * 21); }
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {
@@ -528,8 +557,8 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
     if (subtract) { if (guard) BLTC_GO(RV, OTV, true, true) else BLTC_GO(RV, OTV, true, false) }        \
     else { if (guard) BLTC_GO(RV, OTV, false, true) else BLTC_GO(RV, OTV, false, false) }
     switch (ot) {
-        case 1: BLTC_SG(2, 1)
-        case 2: BLTC_SG(2, 2)
+        case 1: BLTC_SG(BLTC_X_R12, 1)
+        case 2: BLTC_SG(BLTC_X_R12, 2)
         case 3: BLTC_SG(1, 3)
         case 4: BLTC_SG(1, 4)
         default: return cudaErrorInvalidValue;
@@ -538,7 +567,8 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
 #undef BLTC_GO
 }
 
-template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD, 0>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct FarK9 { static auto get() { return far_kernel<R, OT, SUB, GUARD, 9>; } };
 template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD>; } };
 
 cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
@@ -546,6 +576,9 @@ cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items,
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
+    if (degree == 8)          // the paper's n = 8: grid size known at compile time
+        return dispatch_pair<FarK9>(ot, subtract, guard, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
+                                    what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
     return dispatch_pair<FarK>(ot, subtract, guard, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
                                what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
 }
