@@ -41,6 +41,8 @@ UNIT = "interactions/s"
 FLOPS_PER_PAIR = {
     ("near", 1): 34.0, ("near", 2): 50.0, ("near", 3): 66.0, ("near", 4): 82.0,
     ("far", 1): 29.0, ("far", 2): 46.0, ("far", 3): 63.0, ("far", 4): 80.0,
+    # degree 8: far_kernel<..., N1 = 9>, one (k1, k2) row of 9 proxy points per loop trip incl. its dx^2 + dy^2
+    ("far9", 1): 257.0 / 9, ("far9", 2): 410.0 / 9, ("far9", 3): 563.0 / 9, ("far9", 4): 716.0 / 9,
 }
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.
@@ -260,7 +262,8 @@ def run_cuda(args):
         near_ms = phase_sum["near"] / args.steps / len(groups)      # average launch duration
         far_ms = phase_sum["far"] / args.steps / len(groups)
         near_flops = sum(st["near_evals"] * FLOPS_PER_PAIR[("near", g)] for g in groups) / len(groups)
-        far_flops = sum(st["far_evals"] * FLOPS_PER_PAIR[("far", g)] for g in groups) / len(groups)
+        far_key = "far9" if c.degree == 8 else "far"
+        far_flops = sum(st["far_evals"] * FLOPS_PER_PAIR[(far_key, g)] for g in groups) / len(groups)
         peak = FP64_PEAK_TFLOPS_NOMINAL
         near_tf = near_flops / (near_ms * 1e-3) / 1e12
         far_tf = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0

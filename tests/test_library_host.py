@@ -100,7 +100,8 @@ def test_bench_flops_table_matches_the_built_sass():
     rows = [r for r in sass_count.count() if r["SUB"] == 1]
     seen = set()
     for r in rows:                      # every GUARD / ZS variant executes the same FP64 mix per pair
-        key = ("near" if r["kernel"] == "near_kernel" else "far", r["OT"])
+        name = "near" if r["kernel"] == "near_kernel" else ("far9" if r["N1"] == 9 else "far")
+        key = (name, r["OT"])
         assert bench.FLOPS_PER_PAIR[key] == pytest.approx(r["flops"], abs=1e-9), (key, r)
         assert r["R"] == (2 if r["OT"] <= 2 else 1)
         seen.add(key)
