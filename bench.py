@@ -204,7 +204,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     groups = orbital_groups(O)
-    launches_per_step = 5 * len(groups)
+    launches_per_step = int(st["launches_per_group"]) * len(groups)
 
     # ---- device-resident timing -------------------------------------------------------------
     B.bltc_set_profiling(plan, True)

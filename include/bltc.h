@@ -72,6 +72,9 @@ typedef struct bltc_stats {
     int64_t n_far_items;       /* CTAs launched by the far-field kernel (R = 2 tiling) */
     int64_t n_near_items;      /* CTAs launched by the near-field kernel (R = 2 tiling) */
     int64_t partial_len;       /* doubles of partial-sum scratch per orbital */
+    int64_t n_upward_items;    /* CTAs launched by the upward pass (cluster chunks) */
+    int64_t n_upward_reduce;   /* clusters whose chunk-partial proxy charges are summed by a second kernel */
+    int64_t launches_per_group;/* kernels one bltc_convolve launches per orbital group (of <= 4 orbitals) */
     int32_t shared_batches;    /* 1: batches are the source leaves */
     int32_t interp_degree;
     double  theta;

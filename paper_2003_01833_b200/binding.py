@@ -31,7 +31,8 @@ class BltcError(RuntimeError):
 class bltc_stats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in (
         "n_points", "n_clusters", "n_leaves", "n_batches", "n_far", "n_near", "far_evals", "near_evals",
-        "n_proxy_clusters", "upward_pairs", "n_far_items", "n_near_items", "partial_len")] + [
+        "n_proxy_clusters", "upward_pairs", "n_far_items", "n_near_items", "partial_len",
+        "n_upward_items", "n_upward_reduce", "launches_per_group")] + [
         ("shared_batches", C.c_int32), ("interp_degree", C.c_int32),
         ("theta", C.c_double), ("build_ms", C.c_double), ("upload_ms", C.c_double)]
 

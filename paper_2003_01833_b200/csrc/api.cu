@@ -111,6 +111,9 @@ struct bltc_plan_s {
     DevBuf<double> slot_nodes, what;
     DevBuf<Range> near_ranges;
     DevBuf<WorkItem> far_items[2], near_items[2];
+    DevBuf<UpItem> up_items;
+    DevBuf<UpReduce> up_reduce;
+    DevBuf<double> up_chunks;                  // chunk-partial proxy charges (sized for kMaxOT)
     // per-convolve scratch (sized for kMaxOT)
     DevBuf<double> fsrc, ftgt_own, fhat, partial, f_stage, out_stage;
     int last_ot = 0;
@@ -259,8 +262,12 @@ int bltc_create(bltc_handle* h, const double* targets, const double* sources, co
         }
         // f-independent proxy weights what_k (Eq. (35) right with q_j = w_j)
         BLTC_TRY_OR_FREE(pl->what.ensure(ns * (size_t)hp.P));
-        BLTC_TRY_OR_FREE(launch_upward(0, (int)ns, pl->slot_begin.p, pl->slot_end.p, pl->slot_nodes.p,
-                                       hp.degree, pl->src_rec.p, nullptr, pl->what.p, nullptr));
+        BLTC_TRY_OR_FREE(pl->up_items.upload(hp.up_items));
+        BLTC_TRY_OR_FREE(pl->up_reduce.upload(hp.up_reduce));
+        BLTC_TRY_OR_FREE(pl->up_chunks.ensure((size_t)hp.up_partial_chunks * hp.P * kMaxOT));
+        BLTC_TRY_OR_FREE(launch_upward(0, pl->up_items.p, (int)hp.up_items.size(), pl->up_reduce.p,
+                                       (int)hp.up_reduce.size(), pl->slot_nodes.p, hp.degree, pl->src_rec.p,
+                                       nullptr, pl->what.p, pl->up_chunks.p, nullptr));
         BLTC_TRY_OR_FREE(cudaDeviceSynchronize());
     }
 #undef BLTC_TRY_OR_FREE
@@ -293,6 +300,11 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->n_far_items = (int64_t)hp.far_items[1].size();
     s->n_near_items = (int64_t)hp.near_items[1].size();
     s->partial_len = hp.partial_len;
+    s->n_upward_items = (int64_t)hp.up_items.size();
+    s->n_upward_reduce = (int64_t)hp.up_reduce.size();
+    s->launches_per_group = 1 /* gather */ + (hp.shared_order ? 0 : 1) + (hp.up_items.empty() ? 0 : 1) +
+                            (hp.up_reduce.empty() ? 0 : 1) + (hp.far_items[1].empty() ? 0 : 1) +
+                            (hp.near_items[1].empty() ? 0 : 1) + 1 /* epilogue */;
     s->shared_batches = hp.shared_order ? 1 : 0;
     s->interp_degree = hp.degree;
     s->theta = hp.theta;
@@ -428,8 +440,9 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
         }
         if (ev) BLTC_CUDA(cudaEventRecord(ev[1], st));
         // a2: upward pass
-        BLTC_CUDA(launch_upward(ot, (int)ns, h->slot_begin.p, h->slot_end.p, h->slot_nodes.p, hp.degree,
-                                h->src_rec.p, h->fsrc.p, h->fhat.p, st));
+        BLTC_CUDA(launch_upward(ot, h->up_items.p, (int)hp.up_items.size(), h->up_reduce.p,
+                                (int)hp.up_reduce.size(), h->slot_nodes.p, hp.degree, h->src_rec.p, h->fsrc.p,
+                                h->fhat.p, h->up_chunks.p, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
         // a3: far field
         BLTC_CUDA(launch_far(ot, sub, guard, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,

@@ -64,17 +64,18 @@ __global__ void pack_kernel(const double* __restrict__ coords, const double* __r
 }
 
 // ------------------------------------------------------------------------------------ a2
-// One CTA per proxy cluster.  Phase A: barycentric Lagrange values L_k(x_j), L_k(y_j), L_k(z_j)
-// for a tile of particles (Eq. (38)-(39); exact node hits give the unit vector, reading R7).
-// Phase B: every thread owns a (k1, k2) row and 4 consecutive k3 and accumulates
+// One CTA per work item = (proxy cluster, chunk of its particles).  Phase A: barycentric Lagrange
+// values L_k(x_j), L_k(y_j), L_k(z_j) for a tile of particles (Eq. (38)-(39); exact node hits give the
+// unit vector, reading R7).  Phase B: every thread owns a (k1, k2) row and G3 consecutive k3 and accumulates
 //   qhat_k += L_k1 L_k2 L_k3 q_j      (Eq. (35) right)
+// A cluster cut into several chunks is finished by upward_reduce_kernel (chunk order => deterministic).
 constexpr int kUpTile = 64;
 
-template <int OT>
+template <int OT, int G3>
 __global__ void __launch_bounds__(kThreads)
-upward_kernel(const int32_t* __restrict__ slot_begin, const int32_t* __restrict__ slot_end,
-              const double* __restrict__ slot_nodes, int n1, const double4* __restrict__ src_rec,
-              const double* __restrict__ fsrc, double* __restrict__ out) {
+upward_kernel(const UpItem* __restrict__ items, const double* __restrict__ slot_nodes, int n1,
+              const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
+              double* __restrict__ out, double* __restrict__ chunk_out) {
     constexpr int NC = OT == 0 ? 1 : OT;
     extern __shared__ double sm[];
     const int LS = n1 + 3;                       // padded row of L values (pad = 0)
@@ -82,23 +83,24 @@ upward_kernel(const int32_t* __restrict__ slot_begin, const int32_t* __restrict_
     double* s_L = s_nodes + 3 * n1;              // [kUpTile][3][LS]
     double* s_q = s_L + kUpTile * 3 * LS;        // [kUpTile][NC]
     const int tid = threadIdx.x;
-    const int slot = blockIdx.x;
-    const int b = slot_begin[slot], e = slot_end[slot];
+    const UpItem it = items[blockIdx.x];
+    const int slot = it.slot, b = it.begin, e = it.end;
     const int n = n1 - 1;
     const int P = n1 * n1 * n1;
+    double* dst = it.dst < 0 ? out + (size_t)slot * P * NC : chunk_out + (size_t)it.dst * P * NC;
     for (int i = tid; i < 3 * n1; i += kThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
     for (int i = tid; i < kUpTile * 3 * LS; i += kThreads) s_L[i] = 0.0;
-    const int gpr = (n1 + 3) >> 2;               // groups of 4 k3 per (k1, k2) row
+    const int gpr = (n1 + G3 - 1) / G3;          // groups of G3 k3 per (k1, k2) row
     const int units = n1 * n1 * gpr;
     for (int u0 = 0; u0 < units; u0 += kThreads) {
         const int u = u0 + tid;
         const bool active = u < units;
         const int row = active ? u / gpr : 0;
-        const int k3a = active ? (u % gpr) * 4 : 0;
+        const int k3a = active ? (u % gpr) * G3 : 0;
         const int k1 = row / n1, k2 = row % n1;
-        double acc[4][NC];
+        double acc[G3][NC];
 #pragma unroll
-        for (int p = 0; p < 4; ++p)
+        for (int p = 0; p < G3; ++p)
 #pragma unroll
             for (int c = 0; c < NC; ++c) acc[p][c] = 0.0;
         for (int j0 = b; j0 < e; j0 += kUpTile) {
@@ -149,7 +151,7 @@ upward_kernel(const int32_t* __restrict__ slot_begin, const int32_t* __restrict_
 #pragma unroll
                     for (int c = 0; c < NC; ++c) q[c] = s_q[jj * NC + c];
 #pragma unroll
-                    for (int p = 0; p < 4; ++p) {
+                    for (int p = 0; p < G3; ++p) {
                         const double a = a12 * L[2 * LS + k3a + p];
 #pragma unroll
                         for (int c = 0; c < NC; ++c) acc[p][c] = fma(a, q[c], acc[p][c]);
@@ -159,15 +161,27 @@ upward_kernel(const int32_t* __restrict__ slot_begin, const int32_t* __restrict_
         }
         if (active) {
 #pragma unroll
-            for (int p = 0; p < 4; ++p) {
+            for (int p = 0; p < G3; ++p) {
                 const int k3 = k3a + p;
                 if (k3 < n1) {
-                    const size_t kk = (size_t)slot * P + (size_t)(k1 * n1 + k2) * n1 + k3;
+                    const size_t kk = (size_t)(k1 * n1 + k2) * n1 + k3;
 #pragma unroll
-                    for (int c = 0; c < NC; ++c) out[kk * NC + c] = acc[p][c];
+                    for (int c = 0; c < NC; ++c) dst[kk * NC + c] = acc[p][c];
                 }
             }
         }
+    }
+}
+
+// out[slot][i] = sum over the slot's chunks (in chunk order) of chunk_out[first + c][i],  i < P * NC
+__global__ void __launch_bounds__(kThreads)
+upward_reduce_kernel(const UpReduce* __restrict__ red, int len, const double* __restrict__ chunk_out,
+                     double* __restrict__ out) {
+    const UpReduce r = red[blockIdx.y];
+    for (int i = blockIdx.x * kThreads + threadIdx.x; i < len; i += gridDim.x * kThreads) {
+        double s = 0.0;
+        for (int c = 0; c < r.count; ++c) s += chunk_out[(size_t)(r.first + c) * len + i];
+        out[(size_t)r.slot * len + i] = s;
     }
 }
 
@@ -519,26 +533,38 @@ cudaError_t launch_pack_records(const double* coords, const double* w, const int
     return cudaGetLastError();
 }
 
-cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const int32_t* slot_end,
+cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduce* red, int nred,
                           const double* slot_nodes, int degree, const double4* src_rec,
-                          const double* fsrc, double* out, cudaStream_t st) {
-    if (nslot == 0) return cudaSuccess;
+                          const double* fsrc, double* out, double* chunk_out, cudaStream_t st) {
+    if (nitems == 0) return cudaSuccess;
     const int n1 = degree + 1;
     const int nc = ot == 0 ? 1 : ot;
     const size_t smem = sizeof(double) * (3 * n1 + (size_t)kUpTile * 3 * (n1 + 3) + (size_t)kUpTile * nc);
+    const bool g3 = (n1 % 3 == 0) || ((n1 + 2) / 3 * 3 - n1 < (n1 + 3) / 4 * 4 - n1);   // less padding with 3 than with 4
     cudaError_t e = cudaSuccess;
 #define BLTC_UP(OTV)                                                                                   \
     case OTV:                                                                                          \
-        e = set_smem(upward_kernel<OTV>, smem);                                                        \
-        if (e != cudaSuccess) return e;                                                                \
-        upward_kernel<OTV><<<nslot, kThreads, smem, st>>>(slot_begin, slot_end, slot_nodes, n1,        \
-                                                          src_rec, fsrc, out);                         \
+        if (g3) {                                                                                      \
+            e = set_smem(upward_kernel<OTV, 3>, smem);                                                 \
+            if (e != cudaSuccess) return e;                                                            \
+            upward_kernel<OTV, 3><<<nitems, kThreads, smem, st>>>(items, slot_nodes, n1, src_rec,      \
+                                                                   fsrc, out, chunk_out);              \
+        } else {                                                                                       \
+            e = set_smem(upward_kernel<OTV, 4>, smem);                                                 \
+            if (e != cudaSuccess) return e;                                                            \
+            upward_kernel<OTV, 4><<<nitems, kThreads, smem, st>>>(items, slot_nodes, n1, src_rec,      \
+                                                                   fsrc, out, chunk_out);              \
+        }                                                                                              \
         break;
     switch (ot) {
         BLTC_UP(0) BLTC_UP(1) BLTC_UP(2) BLTC_UP(3) BLTC_UP(4)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_UP
+    e = cudaGetLastError();
+    if (e != cudaSuccess || nred == 0) return e;
+    const int len = n1 * n1 * n1 * nc;
+    upward_reduce_kernel<<<dim3((len + kThreads - 1) / kThreads, nred), kThreads, 0, st>>>(red, len, chunk_out, out);
     return cudaGetLastError();
 }
 

@@ -33,10 +33,11 @@ cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const
 cudaError_t launch_pack_records(const double* coords, const double* w, const int32_t* perm, int64_t n,
                                 double4* rec, cudaStream_t st);
 
-// a2: proxy charges.  ot == 0: what[slot][P] from w;  ot >= 1: fhat[slot][P][ot] from f*w
-cudaError_t launch_upward(int ot, int nslot, const int32_t* slot_begin, const int32_t* slot_end,
+// a2: proxy charges.  ot == 0: what[slot][P] from w;  ot >= 1: fhat[slot][P][ot] from f*w.
+// items: chunked work (plan_host.hpp); chunk_out: scratch of up_partial_chunks * P * max(ot,1) doubles
+cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduce* red, int nred,
                           const double* slot_nodes, int degree, const double4* src_rec,
-                          const double* fsrc, double* out, cudaStream_t st);
+                          const double* fsrc, double* out, double* chunk_out, cudaStream_t st);
 
 // a3: far field
 cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,

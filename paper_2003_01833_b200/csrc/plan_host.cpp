@@ -230,6 +230,29 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         }
     }
 
+    // upward-pass work items: clusters are cut into chunks so that ~16 CTAs exist per SM and no CTA
+    // carries a root-level cluster alone; chunk partials are summed in chunk order (deterministic)
+    {
+        const int64_t want = (int64_t)std::max(1, sm_count) * 16;
+        const int64_t chunk = std::min<int64_t>(8192, std::max<int64_t>(512, (p.upward_pairs + want - 1) / want));
+        for (size_t s = 0; s < p.cluster_of_slot.size(); ++s) {
+            const Cluster& C = p.src.cl[p.cluster_of_slot[s]];
+            const int64_t n = C.end - C.begin;
+            const int64_t nch = std::max<int64_t>(1, (n + chunk - 1) / chunk);
+            if (nch == 1) {
+                p.up_items.push_back(UpItem{(int32_t)s, (int32_t)C.begin, (int32_t)C.end, -1});
+                continue;
+            }
+            p.up_reduce.push_back(UpReduce{(int32_t)s, (int32_t)p.up_partial_chunks, (int32_t)nch});
+            for (int64_t c = 0; c < nch; ++c)
+                p.up_items.push_back(UpItem{(int32_t)s, (int32_t)(C.begin + n * c / nch),
+                                            (int32_t)(C.begin + n * (c + 1) / nch), (int32_t)p.up_partial_chunks++});
+        }
+        std::stable_sort(p.up_items.begin(), p.up_items.end(), [](const UpItem& a, const UpItem& c) {
+            return (a.end - a.begin) > (c.end - c.begin);
+        });
+    }
+
     // ---- B200 work decomposition -------------------------------------------------------
     // Per batch: near clusters -> merged contiguous source ranges; far clusters -> slot ids.
     // Lists are cut into segments so that (tiles x segments) gives >= ~32 work items per

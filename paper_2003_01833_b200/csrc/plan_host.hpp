@@ -40,6 +40,12 @@ struct WorkItem {
 struct Range { int32_t begin, end, flags; };
 constexpr int32_t kRangeMayCoincide = 1;
 
+// Upward pass work: one CTA computes the proxy charges of the particle chunk [begin, end) of a slot's
+// cluster.  dst < 0: the slot has a single chunk, the CTA writes the slot's charges directly;
+// dst >= 0: it writes chunk-partial charges number dst, summed afterwards in chunk order (UpReduce).
+struct UpItem { int32_t slot, begin, end, dst; };
+struct UpReduce { int32_t slot, first, count; };
+
 struct HostPlan {
     // parameters
     int64_t N = 0, M = 0;
@@ -65,6 +71,9 @@ struct HostPlan {
     std::vector<int32_t> cluster_of_slot;
     std::vector<double> slot_nodes;            // [nslot][3][degree+1], Eq. (37)
     int64_t upward_pairs = 0;                  // sum over slots of cluster size
+    std::vector<UpItem> up_items;              // chunked upward-pass work, largest first
+    std::vector<UpReduce> up_reduce;           // slots whose chunks must be summed
+    int64_t up_partial_chunks = 0;             // chunk-partial buffers needed (each P * OT doubles)
 
     // device work decomposition
     std::vector<Range> near_ranges;            // merged + cut source ranges, per (batch, segment)
