@@ -42,11 +42,7 @@ __device__ __forceinline__ uint32_t exp_table_init(uint32_t raw, int tid, int nt
         const double v = kExpTab[i];
         // entry j holds the mantissa of 2^(j/T) with the high word pre-biased by -(j << (20 - log2 T)):
         // adding (m << (20 - log2 T)), m = T (n + 1023) + j, then yields 2^n 2^(j/T) with one shift-add
-#ifdef BLTC_X_LOPMERGE
-        const uint32_t hi = (uint32_t)__double2hiint(v);
-#else
         const uint32_t hi = ((uint32_t)__double2hiint(v) & 0x000fffffu) - ((uint32_t)i << (20 - kExpLog2T));
-#endif
         asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(base + 8u * i), "r"((uint32_t)__double2loint(v)), "r"(hi));
     }
     return base;
@@ -108,13 +104,7 @@ __device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, c
     asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
     asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(adr) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8), "r"(tab));   // (a & b) | c
     asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(adr));
-#ifdef BLTC_X_LOPMERGE
-    uint32_t rx, hi2;
-    asm("shf.l.wrap.b32 %0, %1, %1, %2;" : "=r"(rx) : "r"(m), "n"(20 - BLTC_EXP_LOG2T));
-    asm("lop3.b32 %0, %1, %2, %3, 0xE2;" : "=r"(hi2) : "r"(rx), "n"(0x7FF00000), "r"(hi));              // (a & b) | (c & ~b)
-#else
     const uint32_t hi2 = hi + ((uint32_t)m << (20 - BLTC_EXP_LOG2T));       // exponent n + 1023 merged by one shift-add
-#endif
     const double tj = __hiloint2double((int)hi2, (int)lo);   // 2^n * 2^(j/T)
     double p = fma(rho, ec.c3, mr.c2);
     p = fma(p, rho, ec.c1);

@@ -20,26 +20,10 @@
 
 #include "fp64_math.cuh"
 
-// experimental switches (tuning only)
-#ifndef BLTC_X_UNROLL
-#define BLTC_X_UNROLL 2
-#endif
-#ifndef BLTC_X_MINCTAS
-#define BLTC_X_MINCTAS 2
-#endif
-#ifdef BLTC_X_NOZERO
-#define BLTC_X_ZS false
-#else
-#define BLTC_X_ZS true
-#endif
-#ifndef BLTC_X_FUNROLL
-#define BLTC_X_FUNROLL 2
-#endif
-
 namespace bltc {
 namespace {
 
-constexpr int kXUnroll = BLTC_X_UNROLL, kXFUnroll = BLTC_X_FUNROLL;
+constexpr int kNearUnroll = 2, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
@@ -262,7 +246,7 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
                                           const KPar& kp, uint32_t tab, const MathRegs& mr) {
     constexpr int RD = SrcRec<OT>::kDoubles;
     const ExpConst ec{kp.c1, kp.c3};
-#pragma unroll kXUnroll
+#pragma unroll kNearUnroll
     for (int j = j0; j < j1; ++j) {
         const double* s = tile + j * RD;
         const double2 sxy = *reinterpret_cast<const double2*>(s);
@@ -296,7 +280,7 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
 }
 
 template <int R, int OT, bool SUB, bool GUARD>
-__global__ void __launch_bounds__(kThreads, BLTC_X_MINCTAS)
+__global__ void __launch_bounds__(kThreads, 2)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
             const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
@@ -350,7 +334,7 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 : (OT <= 3 ? 4 : 6); };
 
 template <int R, int OT, bool SUB, bool GUARD, int N1>
-__global__ void __launch_bounds__(kThreads, BLTC_X_MINCTAS)
+__global__ void __launch_bounds__(kThreads, 2)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
            const double* __restrict__ fhat, int n1_arg, const double4* __restrict__ tgt_rec,
@@ -359,11 +343,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PD = ProxyRec<OT>::kDoubles;
     static_assert(kProxyTile * PD >= R * OT * 8 * 32, "reduction scratch fits in the tile");
-#ifdef BLTC_X_F9UNROLL
-    constexpr int kU = N1 ? BLTC_X_F9UNROLL : kXFUnroll;
-#else
-    constexpr int kU = N1 ? N1 : kXFUnroll;
-#endif
+    constexpr int kU = N1 ? N1 : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
@@ -583,8 +563,8 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
     if (subtract) { if (guard) BLTC_GO(RV, OTV, true, true) else BLTC_GO(RV, OTV, true, false) }        \
     else { if (guard) BLTC_GO(RV, OTV, false, true) else BLTC_GO(RV, OTV, false, false) }
     switch (ot) {
-        case 1: BLTC_SG(BLTC_X_R12, 1)
-        case 2: BLTC_SG(BLTC_X_R12, 2)
+        case 1: BLTC_SG(2, 1)
+        case 2: BLTC_SG(2, 2)
         case 3: BLTC_SG(1, 3)
         case 4: BLTC_SG(1, 4)
         default: return cudaErrorInvalidValue;

@@ -13,10 +13,7 @@ constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (nea
 constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field)
 
 // targets per thread for an orbital tile of width ot
-#ifndef BLTC_X_R12
-#define BLTC_X_R12 2
-#endif
-inline int targets_per_thread(int ot) { return ot <= 2 ? BLTC_X_R12 : 1; }
+inline int targets_per_thread(int ot) { return ot <= 2 ? 2 : 1; }
 
 // per-orbital constants of the tile (kernel parameter -> constant bank):
 //   nk = -k_o;  c = -k_o T/ln2 (scaled exponent argument of fp64_math.cuh's exp);  c1, c3: polynomial
