@@ -463,3 +463,90 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
     free(fhat); free(what); free(fw); free(need);
     return 0;
 }
+
+/* ------------------------------------------------------------------ evaluation, Coulomb kernel
+ * Hartree potential (Eq. (19)) through the same treecode, with the Gaussian singularity
+ * subtraction of PAPER.md:220-224 Eq. (23)-(24) (O-3 in DESIGN.md; direct definition in
+ * oracle/coulomb_sum.c).  "Singularity subtraction ... can be easily accommodated in the BLTC"
+ * -- not shown; reading R21: the first integrand of Eq. (23) is the sum of two
+ * convolutions, kernel 1/r with charges f_j w_j and kernel e^{-r^2/alpha^2}/r with charges w_j
+ * (times -f_i), and each is approximated by Eq. (35) with its own proxy charges:
+ *   far  = sum_k [ fhat_k / |x_i - s_k|  -  f_i what_k e^{-|x_i - s_k|^2/alpha^2} / |x_i - s_k| ]
+ *   near = sum_{r_j in C, r_ij != 0} (f_j - f_i e^{-r_ij^2/alpha^2}) w_j / r_ij          (Eq. (34))
+ *   V_i  = far + near + 2 pi alpha^2 f_i                                               (Eq. (24))
+ * Same lists, same proxy charges, same order of the sums as oracle_bltc_eval. */
+double oracle_coulomb_term(double tx, double ty, double tz, double sx, double sy, double sz,
+                           double fi, double fj, double wj, double alpha, int subtract, int* skip);  /* oracle/coulomb_sum.c */
+
+int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double* f_src,
+                             const double* f_tgt, double alpha, int subtract,
+                             int64_t nsel, const int64_t* sel, double* out, double* parts)
+{
+    if (!p || !w || !f_src || !out) return -1;
+    if (subtract && (!f_tgt || !(alpha > 0.0))) return -1;
+    int n1 = p->degree + 1, P = p->P, ncl = p->src.ncl;
+    int64_t nb = sel ? nsel : p->nbatch;
+    char* need = (char*)calloc((size_t)ncl, 1);
+    for (int64_t s = 0; s < nb; ++s) {
+        int64_t b = sel ? sel[s] : s;
+        if (b < 0 || b >= p->nbatch) { free(need); return -1; }
+        for (int64_t q = p->far_ptr[b]; q < p->far_ptr[b + 1]; ++q) need[p->far.v[q]] = 1;
+    }
+    double** fhat = (double**)calloc((size_t)ncl, sizeof(double*));
+    double** what = (double**)calloc((size_t)ncl, sizeof(double*));
+    double* fw = (double*)malloc((size_t)p->N * sizeof(double));
+    for (int64_t j = 0; j < p->N; ++j) fw[j] = f_src[j] * w[j];
+    int c;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (c = 0; c < ncl; ++c) {
+        if (!need[c]) continue;
+        fhat[c] = (double*)malloc((size_t)P * sizeof(double));
+        proxy_charges(p, c, fw, fhat[c]);
+        if (subtract) { what[c] = (double*)malloc((size_t)P * sizeof(double)); proxy_charges(p, c, w, what[c]); }
+    }
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (s = 0; s < nb; ++s) {
+        int64_t b = sel ? sel[s] : s;
+        for (int64_t it = p->bbegin[b]; it < p->bend[b]; ++it) {
+            int64_t i = p->tperm[it];
+            double xi = p->tx[i], yi = p->ty[i], zi = p->tz[i];
+            double fi = subtract ? f_tgt[i] : 0.0;
+            long double Sfar = 0.0L, Snear = 0.0L;
+            for (int64_t q = p->far_ptr[b]; q < p->far_ptr[b + 1]; ++q) {
+                int cc = p->far.v[q];
+                const double* sn = p->nodes + (size_t)cc * 3 * n1;
+                for (int k1 = 0; k1 < n1; ++k1)
+                    for (int k2 = 0; k2 < n1; ++k2)
+                        for (int k3 = 0; k3 < n1; ++k3) {
+                            int kk = (k1 * n1 + k2) * n1 + k3;
+                            double dx = xi - sn[k1], dy = yi - sn[n1 + k2], dz = zi - sn[2 * n1 + k3];
+                            double r2 = dx * dx + dy * dy + dz * dz;
+                            double r = sqrt(r2);
+                            if (r == 0.0) continue;
+                            double t = fhat[cc][kk] / r;
+                            if (subtract) t -= fi * what[cc][kk] * exp(-r2 / (alpha * alpha)) / r;
+                            Sfar += (long double)t;
+                        }
+            }
+            for (int64_t q = p->near_ptr[b]; q < p->near_ptr[b + 1]; ++q) {
+                const cluster_t* C = &p->src.cl[p->near.v[q]];
+                for (int64_t jt = C->begin; jt < C->end; ++jt) {
+                    int64_t j = p->src.perm[jt];
+                    int skip;
+                    double t = oracle_coulomb_term(xi, yi, zi, p->sx[j], p->sy[j], p->sz[j], fi, f_src[j], w[j],
+                                                   alpha, subtract, &skip);
+                    if (skip) continue;
+                    Snear += (long double)t;
+                }
+            }
+            long double S = Sfar + Snear;
+            if (parts) { parts[i] = (double)Sfar; parts[p->M + i] = (double)Snear; }
+            if (subtract) S += 2.0L * (long double)M_PI * (long double)alpha * (long double)alpha * (long double)fi;
+            out[i] = (double)S;
+        }
+    }
+    for (c = 0; c < ncl; ++c) { free(fhat[c]); free(what[c]); }
+    free(fhat); free(what); free(fw); free(need);
+    return 0;
+}

@@ -12,7 +12,7 @@ import sys
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, "direct_sum.c"), os.path.join(_HERE, "bltc_cpu.c")]
+_SRC = [os.path.join(_HERE, "direct_sum.c"), os.path.join(_HERE, "coulomb_sum.c"), os.path.join(_HERE, "bltc_cpu.c")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 # strict IEEE: no fast-math, no FMA contraction, baseline x86-64 (no -march=native)
 _CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
@@ -57,6 +57,12 @@ def _load():
     lib.oracle_bltc_eval.restype = C.c_int
     lib.oracle_bltc_eval.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_double, C.c_int, C.c_int,
                                      C.c_int64, _ip64, _dp, _dp]
+    lib.oracle_coulomb_direct.restype = C.c_int
+    lib.oracle_coulomb_direct.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, C.c_int64, _dp, _dp, _dp, _dp, _dp,
+                                          C.c_double, C.c_int, _dp]
+    lib.oracle_bltc_eval_coulomb.restype = C.c_int
+    lib.oracle_bltc_eval_coulomb.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_double, C.c_int,
+                                             C.c_int64, _ip64, _dp, _dp]
     _lib = lib
     return lib
 
@@ -108,6 +114,37 @@ def direct(targets, sources, w, f_src, k, *, f_tgt=None, subtract=True, finalize
                                float(K[o]), int(subtract), int(finalize), oo.ctypes.data_as(_dp))
         if rc != 0:
             raise ValueError("oracle_direct: bad arguments")
+        out[o] = oo
+    return out[0] if single else out
+
+
+def coulomb_direct(targets, sources, w, f_src, *, f_tgt=None, subtract=True, alpha=1.0):
+    """Hartree-potential direct sum with Gaussian singularity subtraction (oracle/coulomb_sum.c,
+    PAPER.md:197-224 Eq. (19),(23),(24)).  f_src: [N] or [n_f][N].  Returns [M] or [n_f][M]."""
+    lib = _load()
+    tx, ptx = _d(targets[0]); ty, pty = _d(targets[1]); tz, ptz = _d(targets[2])
+    sx, psx = _d(sources[0]); sy, psy = _d(sources[1]); sz, psz = _d(sources[2])
+    w_, pw = _d(w)
+    f_src = np.asarray(f_src, dtype=np.float64)
+    single = f_src.ndim == 1
+    F = np.atleast_2d(f_src)
+    FT = None
+    if subtract:
+        if f_tgt is None:
+            raise ValueError("subtract=True needs f_tgt (f at the targets)")
+        FT = np.atleast_2d(np.asarray(f_tgt, dtype=np.float64))
+    M, N = tx.shape[0], sx.shape[0]
+    out = np.empty((F.shape[0], M))
+    for o in range(F.shape[0]):
+        fo, pfo = _d(F[o])
+        pfto = None
+        if subtract:
+            fto, pfto = _d(FT[o])
+        oo = np.empty(M)
+        rc = lib.oracle_coulomb_direct(M, ptx, pty, ptz, pfto, N, psx, psy, psz, pw, pfo,
+                                       float(alpha), int(subtract), oo.ctypes.data_as(_dp))
+        if rc != 0:
+            raise ValueError("oracle_coulomb_direct: bad arguments")
         out[o] = oo
     return out[0] if single else out
 
@@ -212,6 +249,47 @@ class OraclePlan:
                                             pp.ctypes.data_as(_dp) if return_parts else None)
             if rc != 0:
                 raise ValueError("oracle_bltc_eval: bad arguments")
+            out[o] = oo
+            if return_parts:
+                parts[o] = pp
+        res = out[0] if single else out
+        if return_parts:
+            return res, (parts[0] if single else parts)
+        return res
+
+    def evaluate_coulomb(self, w, f_src, *, f_tgt=None, subtract=True, alpha=1.0, batches=None,
+                         return_parts=False):
+        """Hartree potential through the treecode (oracle_bltc_eval_coulomb, reading R21)."""
+        w_, pw = _d(w)
+        f_src = np.asarray(f_src, dtype=np.float64)
+        single = f_src.ndim == 1
+        F = np.atleast_2d(f_src)
+        if subtract:
+            if f_tgt is None:
+                if self._t is not None:
+                    raise ValueError("subtract with separate targets needs f_tgt")
+                FT = F
+            else:
+                FT = np.atleast_2d(np.asarray(f_tgt, dtype=np.float64))
+        if batches is not None:
+            sel = np.ascontiguousarray(batches, dtype=np.int64)
+            nsel, psel = sel.shape[0], sel.ctypes.data_as(_ip64)
+        else:
+            nsel, psel = 0, None
+        out = np.full((F.shape[0], self.M), np.nan)
+        parts = np.full((F.shape[0], 2, self.M), np.nan) if return_parts else None
+        for o in range(F.shape[0]):
+            fo, pfo = _d(F[o])
+            pft = None
+            if subtract:
+                fto, pft = _d(FT[o])
+            oo = np.full(self.M, np.nan)
+            pp = np.full((2, self.M), np.nan) if return_parts else None
+            rc = self._lib.oracle_bltc_eval_coulomb(self._h, pw, pfo, pft, float(alpha), int(subtract),
+                                                    nsel, psel, oo.ctypes.data_as(_dp),
+                                                    pp.ctypes.data_as(_dp) if return_parts else None)
+            if rc != 0:
+                raise ValueError("oracle_bltc_eval_coulomb: bad arguments")
             out[o] = oo
             if return_parts:
                 parts[o] = pp
