@@ -43,6 +43,10 @@ FLOPS_PER_PAIR = {
     ("far", 1): 29.0, ("far", 2): 46.0, ("far", 3): 63.0, ("far", 4): 80.0,
     # degree 8: far_kernel<..., N1 = 9>, one (k1, k2) row of 9 proxy points per loop trip incl. its dx^2 + dy^2
     ("far9", 1): 257.0 / 9, ("far9", 2): 410.0 / 9, ("far9", 3): 563.0 / 9, ("far9", 4): 716.0 / 9,
+    # Coulomb kernel with Gaussian singularity subtraction (bltc_convolve_coulomb)
+    ("cnear", 1): 33.0, ("cnear", 2): 37.0, ("cnear", 3): 41.0, ("cnear", 4): 45.0,
+    ("cfar", 1): 28.0, ("cfar", 2): 32.0, ("cfar", 3): 36.0, ("cfar", 4): 40.0,
+    ("cfar9", 1): 248.0 / 9, ("cfar9", 2): 284.0 / 9, ("cfar9", 3): 320.0 / 9, ("cfar9", 4): 356.0 / 9,
 }
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.
@@ -108,12 +112,25 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload():
+def workload(name="cfg1", kernel="yukawa"):
+    """cfg1 (BASELINE.json configs[1]) is the bench workload; the others are for profiling and context runs.
+    kernel = "coulomb": the same mesh with ONE field, the density rho = 2 sum_o psi_o^2 -- the Hartree
+    potential of bltc_convolve_coulomb (Table 4's workload shape)."""
     from paper_2003_01833_b200 import inputs as I
-    return I.config1()
+    c = {"cfg0": I.config0, "cfg1": I.config1, "cfg2": I.config2, "cfg3": I.config3}[name]()
+    if kernel == "coulomb":
+        c = I.density_workload(c)
+    return c
 
 
-def cpu_oracle_sample(c, batches, repeat=1):
+def sample_batches(n_batches, count=4):
+    """Evenly spread batch ids; cfg1 (568 batches) keeps the ids the earlier rounds used."""
+    if n_batches == 568:
+        return [0, 137, 301, 567][:count]
+    return sorted(set(int(round(i * (n_batches - 1) / max(count - 1, 1))) for i in range(count)))
+
+
+def cpu_oracle_sample(c, batches, repeat=1, kernel="yukawa"):
     """Time the CPU oracle's BLTC (as it stands) on a bounded sample of target batches and scale to the
     whole convolution by evaluation count.  Returns (equiv. interactions/s, seconds, description)."""
     import oracle
@@ -121,6 +138,8 @@ def cpu_oracle_sample(c, batches, repeat=1):
     e = op.export()
     size = e["cl_end"] - e["cl_begin"]
     ev = 0
+    if isinstance(batches, int):
+        batches = sample_batches(op.n_batches, batches)
     for b in batches:
         nt = e["b_end"][b] - e["b_begin"][b]
         ev += nt * (op.P * (e["far_ptr"][b + 1] - e["far_ptr"][b])
@@ -129,7 +148,10 @@ def cpu_oracle_sample(c, batches, repeat=1):
     best = None
     for _ in range(repeat):
         t0 = time.perf_counter()
-        op.evaluate(c.w, c.f, c.k, batches=list(batches))
+        if kernel == "coulomb":
+            op.evaluate_coulomb(c.w, c.f, alpha=1.0, batches=list(batches))
+        else:
+            op.evaluate(c.w, c.f, c.k, batches=list(batches))
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     t_full = best * total / ev                       # seconds for all batches, all orbitals
@@ -146,11 +168,11 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    c = workload()
-    batches = [137]
+    c = workload(args.workload, args.kernel)
+    batches = [137] if args.workload == "cfg1" else 1
     vals = []
     for i in range(args.warmup + args.steps):
-        v, dt, desc, cores = cpu_oracle_sample(c, batches)
+        v, dt, desc, cores = cpu_oracle_sample(c, batches, kernel=args.kernel)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
@@ -185,14 +207,26 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
 
-    c = workload()
+    c = workload(args.workload, args.kernel)
+    coulomb = args.kernel == "coulomb"
     N, O = c.N, c.n_orb
+
+    def convolve(f_, out_):
+        if coulomb:
+            B.bltc_convolve_coulomb(plan, f_, O, out_, True, 1.0)
+        else:
+            B.bltc_convolve(plan, c.k, f_, O, out_, True)
+
     X = torch.from_numpy(c.coords()).cuda()
     w = torch.from_numpy(c.w).cuda()
     f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
-    out = torch.empty((O, N), dtype=torch.float64, device="cuda")
+    out = torch.zeros((O, N), dtype=torch.float64, device="cuda")      # a sharded plan writes its slice only
     t0 = time.perf_counter()
-    plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    sharded = args.shard == "batches" and world > 1
+    if sharded:      # strong scaling: rank r computes its slice of the target batches, no collective
+        plan = B.bltc_create_sharded(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
+    else:
+        plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
     create_ms = (time.perf_counter() - t0) * 1e3
     st = B.bltc_get_stats(plan)
     stream = torch.cuda.current_stream()
@@ -209,7 +243,7 @@ def run_cuda(args):
     # ---- device-resident timing -------------------------------------------------------------
     B.bltc_set_profiling(plan, True)
     for _ in range(max(args.warmup, 3)):
-        B.bltc_convolve(plan, c.k, f, O, out, True)
+        convolve(f, out)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -219,7 +253,7 @@ def run_cuda(args):
     for i in range(args.steps):
         flush.fill_(0.0)                                        # L2 flush between timed iterations
         ev[i][0].record(stream)
-        B.bltc_convolve(plan, c.k, f, O, out, True)
+        convolve(f, out)
         ev[i][1].record(stream)
         ph = B.bltc_get_phase_ms(plan)                          # syncs on the step's last event
         for p in B.PHASES:
@@ -232,21 +266,22 @@ def run_cuda(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         t_ms = float(t.item())
     ms_per_step = t_ms / args.steps
-    value = world * O * float(N) ** 2 / (ms_per_step * 1e-3)
+    jobs = 1 if sharded else world          # replicas: every rank convolves its own orbitals on the same mesh
+    value = jobs * O * float(N) ** 2 / (ms_per_step * 1e-3)
 
     # ---- end to end through the C ABI with host buffers ------------------------------------
     B.bltc_set_profiling(plan, False)
     f_host = torch.from_numpy(np.ascontiguousarray(c.f)).pin_memory()
-    out_host = torch.empty((O, N), dtype=torch.float64).pin_memory()
+    out_host = torch.zeros((O, N), dtype=torch.float64).pin_memory()
     for _ in range(2):
-        B.bltc_convolve(plan, c.k, f_host, O, out_host, True)
+        convolve(f_host, out_host)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e2e_ms = 0.0
     for i in range(args.steps):
         flush.fill_(0.0)
         e0.record(stream)
-        B.bltc_convolve(plan, c.k, f_host, O, out_host, True)   # H2D(f) + a1..a5 + D2H(out) + stream sync
+        convolve(f_host, out_host)                              # H2D(f) + a1..a5 + D2H(out) + stream sync
         e1.record(stream)
         e1.synchronize()
         e2e_ms += e0.elapsed_time(e1)
@@ -255,37 +290,48 @@ def run_cuda(args):
         t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item())
-    e2e_value = world * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
+    e2e_value = jobs * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
     same = bool(np.array_equal(out_host.numpy(), out.cpu().numpy()))
 
     if rank == 0:
         near_ms = phase_sum["near"] / args.steps / len(groups)      # average launch duration
         far_ms = phase_sum["far"] / args.steps / len(groups)
-        near_flops = sum(st["near_evals"] * FLOPS_PER_PAIR[("near", g)] for g in groups) / len(groups)
-        far_key = "far9" if c.degree == 8 else "far"
+        pre = "c" if coulomb else ""
+        if sharded:                          # rank 0's kernels work on rank 0's slice
+            st = dict(st, near_evals=st["shard_near_evals"], far_evals=st["shard_far_evals"])
+        near_flops = sum(st["near_evals"] * FLOPS_PER_PAIR[(pre + "near", g)] for g in groups) / len(groups)
+        far_key = pre + ("far9" if c.degree == 8 else "far")
         far_flops = sum(st["far_evals"] * FLOPS_PER_PAIR[(far_key, g)] for g in groups) / len(groups)
         peak = FP64_PEAK_TFLOPS_NOMINAL
         near_tf = near_flops / (near_ms * 1e-3) / 1e12
         far_tf = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
         probe = B.bltc_probe_fp64(64)
+        # DRAM bytes of one near-kernel launch of THIS workload from the committed ncu capture
+        # (profiles/r01c_near_kernel_ncu.md names the command); null for other workloads / kernels
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r01_near_traffic.json")
-        if os.path.exists(tpath):
+        tpath = os.path.join(ROOT, "profiles", "r01c_near_cfg1_dram.csv")
+        if args.workload == "cfg1" and not coulomb and os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+                import csv
+                rows = [r for r in csv.reader(open(tpath)) if len(r) > 5 and r[-3].startswith("dram__bytes")]
+                traffic = float(sum(float(r[-1].replace(",", "")) for r in rows)) if rows else None
             except Exception:
                 traffic = None
-        cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, [0, 137, 301, 567])
+        cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, 4, kernel=args.kernel)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": c.name + " (BASELINE.json configs[1])", "N": N, "n_orb": O, "theta": c.theta,
+            "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c.name + (" (BASELINE.json configs[1])" if args.workload == "cfg1" and not coulomb else ""),
+                       "kernel": "coulomb 1/r, Gaussian subtraction alpha = 1 (Eq. (23)-(24))" if coulomb
+                       else "yukawa e^{-kr}/(4 pi r), subtraction Eq. (20)-(21)", "N": N, "n_orb": O, "theta": c.theta,
                        "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
                        "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                       "parallelism": ("1 GPU" if world == 1 else
+                                       f"target batches sharded over {world} ranks, no collective" if sharded
+                                       else f"{world} replicas (each rank its own orbitals), no collective")},
             "time_per_convolution_ms": ms_per_step / O,
-            "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O / (ms_per_step * 1e-3),
+            "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * world / (ms_per_step * 1e-3),
             "phase_ms": {p: phase_sum[p] / args.steps for p in B.PHASES},
             "plan": {"create_ms": create_ms, "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
                      "clusters": st["n_clusters"], "batches": st["n_batches"],
@@ -318,6 +364,13 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "batches"],
+                    help="N > 1: replicas = each rank convolves its own orbitals (weak scaling, default); "
+                         "batches = one convolution, target batches sharded over the ranks (strong scaling)")
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"],
+                    help="cfg1 = BASELINE.json configs[1] (the bench line); others: profiling / context")
+    ap.add_argument("--kernel", default="yukawa", choices=["yukawa", "coulomb"],
+                    help="coulomb: Hartree potential with Gaussian singularity subtraction (NEXT-1)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -80,6 +80,13 @@ typedef struct bltc_stats {
     double  theta;
     double  build_ms;          /* host wall-clock of tree + lists + work decomposition */
     double  upload_ms;         /* host wall-clock of device upload + f-independent proxy weights */
+    /* batch sharding (bltc_create_sharded); an unsharded plan reports rank 0 of 1 and all batches */
+    int32_t shard_rank, shard_world;
+    int64_t shard_batch_begin; /* this plan computes the batches [begin, end) ... */
+    int64_t shard_batch_end;
+    int64_t shard_targets;     /* ... = this many targets (a contiguous range in target tree order) */
+    int64_t shard_far_evals;   /* kernel evaluations per orbital of this plan's batches */
+    int64_t shard_near_evals;
 } bltc_stats;
 
 /* Phases of one bltc_convolve, for bltc_get_phase_ms (device times, CUDA events on `stream`). */
@@ -99,6 +106,25 @@ enum { BLTC_PHASE_GATHER = 0, BLTC_PHASE_UPWARD = 1, BLTC_PHASE_FAR = 2, BLTC_PH
  */
 int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                 int64_t N, double theta, int interp_degree, int batch_size, int leaf_size);
+
+/*
+ * Multi-GPU batch sharding (the paper's multi-GPU split, PAPER.md:494-500:
+ * "the compute stage has close to ideal scaling").  Target batches are independent given the sources and the
+ * proxy charges, so rank r of `world` builds the SAME tree, batches and lists (the whole problem's: every rank
+ * holds all sources) and keeps the device work of a contiguous slice of the batch list that carries ~1/world of
+ * the far + near kernel evaluations; proxy charges are computed (redundantly, ~0.5 % of the work) only for the
+ * clusters its own far lists use.  No data-path collective is needed: bltc_convolve / bltc_convolve_coulomb on
+ * such a plan write out[o][i] ONLY for the targets i of the plan's batches and leave every other element of
+ * `out` untouched; bltc_get_shard_targets lists those i (caller's point indices, `shard_targets` of them, in
+ * target tree order).  Slices of different ranks are disjoint and cover all targets.  world = 1 is bltc_create.
+ */
+int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                        int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
+                        int rank, int world);
+int bltc_create_host_plan_sharded(bltc_handle* h, const double* targets, const double* sources,
+                                  const double* weights, int64_t N, double theta, int interp_degree,
+                                  int batch_size, int leaf_size, int rank, int world);
+int bltc_get_shard_targets(bltc_handle h, int64_t* idx /* HOST int64[shard_targets] */);
 
 /* Same plan, host part only (no CUDA call is made): for structural inspection through
  * bltc_get_stats / bltc_export_plan.  weights may be NULL.  bltc_convolve on such a handle
@@ -130,6 +156,30 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
                     const double* sources, const double* weights, const double* f_sources, int64_t N,
                     const double* k, int n_orb, double* out, int subtract_singularity,
                     bltc_stream stream);
+
+/*
+ * the Hartree potential (Eq. (19)) through the same plan: Coulomb kernel
+ * 1/r with the Gaussian singularity subtraction of PAPER.md:220-224 Eq. (23)-(24) ("alpha = 1 a.u.",
+ * PAPER.md:229).  This is the convolution the paper times in Table 4 and Fig. 11.
+ *
+ *   subtract_singularity = 1:
+ *     out[o][i] = sum_{j : r_ij != 0} (f[o][j] - f[o][i] e^{-r_ij^2/alpha^2}) w_j / r_ij  +  2 pi alpha^2 f[o][i]
+ *   subtract_singularity = 0:
+ *     out[o][i] = sum_{j : r_ij != 0} f[o][j] w_j / r_ij                      (alpha ignored)
+ *
+ * No 1/(4 pi) and no -2: the kernel of Eq. (19) as printed.  The treecode approximates the first integrand of
+ * Eq. (23) as two interpolated convolutions (reading R21): far field
+ *     sum_k [ fhat_k - f_i what_k e^{-|x_i - s_k|^2/alpha^2} ] / |x_i - s_k|.
+ * f, out: double[n_f][N] in the caller's point order (n_f densities share every kernel evaluation);
+ * pointers, stream and error conventions as bltc_convolve / direct_convolve.  alpha > 0 (and
+ * alpha > 2e-6 x the domain diameter) when subtract_singularity = 1.
+ */
+int bltc_convolve_coulomb(bltc_handle h, const double* f, int n_f, double* out, int subtract_singularity,
+                          double alpha, bltc_stream stream);
+
+int direct_convolve_coulomb(const double* targets, const double* f_targets, int64_t M,
+                            const double* sources, const double* weights, const double* f_sources, int64_t N,
+                            int n_f, double* out, int subtract_singularity, double alpha, bltc_stream stream);
 
 int bltc_destroy(bltc_handle h);
 

@@ -34,10 +34,14 @@ class bltc_stats(C.Structure):
         "n_proxy_clusters", "upward_pairs", "n_far_items", "n_near_items", "partial_len",
         "n_upward_items", "n_upward_reduce", "launches_per_group")] + [
         ("shared_batches", C.c_int32), ("interp_degree", C.c_int32),
-        ("theta", C.c_double), ("build_ms", C.c_double), ("upload_ms", C.c_double)]
+        ("theta", C.c_double), ("build_ms", C.c_double), ("upload_ms", C.c_double),
+        ("shard_rank", C.c_int32), ("shard_world", C.c_int32)] + [(n, C.c_int64) for n in (
+            "shard_batch_begin", "shard_batch_end", "shard_targets", "shard_far_evals", "shard_near_evals")]
 
 
-EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_convolve", "direct_convolve", "bltc_destroy",
+EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
+            "bltc_get_shard_targets", "bltc_convolve", "direct_convolve",
+            "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
             "bltc_probe_fp64", "bltc_last_error", "bltc_version")
@@ -57,8 +61,14 @@ def lib():
     L.bltc_version.restype = C.c_char_p
     L.bltc_create.argtypes = [C.POINTER(vp), vp, vp, vp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_int]
     L.bltc_create_host_plan.argtypes = L.bltc_create.argtypes
+    L.bltc_create_sharded.argtypes = L.bltc_create.argtypes + [C.c_int, C.c_int]
+    L.bltc_create_host_plan_sharded.argtypes = L.bltc_create_sharded.argtypes
+    L.bltc_get_shard_targets.argtypes = [vp, _i64p]
     L.bltc_convolve.argtypes = [vp, _dp, vp, C.c_int, vp, C.c_int, vp]
     L.direct_convolve.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, _dp, C.c_int, vp, C.c_int, vp]
+    L.bltc_convolve_coulomb.argtypes = [vp, vp, C.c_int, vp, C.c_int, C.c_double, vp]
+    L.direct_convolve_coulomb.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, C.c_int, vp, C.c_int,
+                                          C.c_double, vp]
     L.bltc_destroy.argtypes = [vp]
     L.bltc_get_stats.argtypes = [vp, C.POINTER(bltc_stats)]
     L.bltc_export_plan.argtypes = [vp, _i64p, _i64p, _i64p, _i64p, _dp, _dp, _i32p, _i32p, _i64p, _i64p,
@@ -137,12 +147,32 @@ class Plan:
             pass
 
 
-def _create(fn, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
+def _create(fn, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, *shard):
     h = C.c_void_p()
     _check(fn(C.byref(h), _ptr(targets, "targets", True), _ptr(sources, "sources"),
               _ptr(weights, "weights", True), int(N), float(theta), int(interp_degree),
-              int(batch_size), int(leaf_size)))
+              int(batch_size), int(leaf_size), *[int(v) for v in shard]))
     return Plan(h, int(N))
+
+
+def bltc_create_sharded(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, rank, world):
+    """include/bltc.h bltc_create_sharded: rank's slice of the target batches (multi-GPU, no collective)."""
+    return _create(lib().bltc_create_sharded, targets, sources, weights, N, theta, interp_degree, batch_size,
+                   leaf_size, rank, world)
+
+
+def bltc_create_host_plan_sharded(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size,
+                                  rank, world):
+    return _create(lib().bltc_create_host_plan_sharded, targets, sources, weights, N, theta, interp_degree,
+                   batch_size, leaf_size, rank, world)
+
+
+def bltc_get_shard_targets(plan):
+    """Caller indices of the targets a (sharded) plan computes, in target tree order."""
+    n = bltc_get_stats(plan)["shard_targets"]
+    idx = np.empty(n, dtype=np.int64)
+    _check(lib().bltc_get_shard_targets(plan._h, idx.ctypes.data_as(_i64p)))
+    return idx
 
 
 def bltc_create(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
@@ -171,6 +201,23 @@ def direct_convolve(targets, f_targets, M, sources, weights, f_sources, N, k, n_
                                  _ptr(sources, "sources"), _ptr(weights, "weights"),
                                  _ptr(f_sources, "f_sources"), int(N), kk.ctypes.data_as(_dp), int(n_orb),
                                  _ptr(out, "out"), int(bool(subtract_singularity)), _stream_ptr(stream)))
+    return out
+
+
+def bltc_convolve_coulomb(plan, f, n_f, out, subtract_singularity=True, alpha=1.0, stream=None):
+    """include/bltc.h bltc_convolve_coulomb (Hartree potential, Gaussian singularity subtraction)."""
+    _check(lib().bltc_convolve_coulomb(plan._h, _ptr(f, "f"), int(n_f), _ptr(out, "out"),
+                                       int(bool(subtract_singularity)), float(alpha), _stream_ptr(stream)))
+    return out
+
+
+def direct_convolve_coulomb(targets, f_targets, M, sources, weights, f_sources, N, n_f, out,
+                            subtract_singularity=True, alpha=1.0, stream=None):
+    """include/bltc.h direct_convolve_coulomb."""
+    _check(lib().direct_convolve_coulomb(_ptr(targets, "targets"), _ptr(f_targets, "f_targets", True), int(M),
+                                         _ptr(sources, "sources"), _ptr(weights, "weights"),
+                                         _ptr(f_sources, "f_sources"), int(N), int(n_f), _ptr(out, "out"),
+                                         int(bool(subtract_singularity)), float(alpha), _stream_ptr(stream)))
     return out
 
 

@@ -138,9 +138,9 @@ int check_create_args(bltc_handle* h, const double* sources, int64_t N, double t
 }
 
 int build_plan_guarded(bltc_plan_s* pl, const double* targets, const double* sources, int64_t N,
-                       double theta, int degree, int batch_size, int leaf_size, int sms) {
+                       double theta, int degree, int batch_size, int leaf_size, int sms, int rank, int world) {
     try {
-        build_host_plan(pl->hp, targets, sources, N, theta, degree, batch_size, leaf_size, sms);
+        build_host_plan(pl->hp, targets, sources, N, theta, degree, batch_size, leaf_size, sms, rank, world);
     } catch (const std::bad_alloc&) {
         return fail(BLTC_ENOMEM, "host allocation failed while building the plan");
     } catch (const std::exception& e) {
@@ -162,24 +162,39 @@ extern "C" {
 const char* bltc_last_error(void) { return g_err.c_str(); }
 const char* bltc_version(void) { return "bltc-b200 0.1 (sm_100a)"; }
 
-int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* sources,
-                          const double* weights, int64_t N, double theta, int interp_degree,
-                          int batch_size, int leaf_size) {
+int bltc_create_host_plan_sharded(bltc_handle* h, const double* targets, const double* sources,
+                                  const double* weights, int64_t N, double theta, int interp_degree,
+                                  int batch_size, int leaf_size, int rank, int world) {
     (void)weights;
     int rc = check_create_args(h, sources, N, theta, interp_degree, batch_size, leaf_size);
     if (rc) return rc;
+    if (world < 1 || rank < 0 || rank >= world) return fail(BLTC_EINVAL, "need 0 <= rank < world");
     bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
     if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
-    rc = build_plan_guarded(pl, targets, sources, N, theta, interp_degree, batch_size, leaf_size, 148);
+    rc = build_plan_guarded(pl, targets, sources, N, theta, interp_degree, batch_size, leaf_size, 148, rank, world);
     if (rc) { delete pl; return rc; }
     *h = pl;
     return BLTC_OK;
 }
 
+int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* sources,
+                          const double* weights, int64_t N, double theta, int interp_degree,
+                          int batch_size, int leaf_size) {
+    return bltc_create_host_plan_sharded(h, targets, sources, weights, N, theta, interp_degree, batch_size,
+                                         leaf_size, 0, 1);
+}
+
 int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                 int64_t N, double theta, int interp_degree, int batch_size, int leaf_size) {
+    return bltc_create_sharded(h, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, 0, 1);
+}
+
+int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                        int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
+                        int rank, int world) {
     int rc = check_create_args(h, sources, N, theta, interp_degree, batch_size, leaf_size);
     if (rc) return rc;
+    if (world < 1 || rank < 0 || rank >= world) return fail(BLTC_EINVAL, "need 0 <= rank < world");
     if (!weights) return fail(BLTC_EINVAL, "weights is NULL");
     int dev = 0, sms = 0;
     BLTC_CUDA(cudaGetDevice(&dev));
@@ -199,7 +214,7 @@ int bltc_create(bltc_handle* h, const double* targets, const double* sources, co
     bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
     if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
     rc = build_plan_guarded(pl, same ? nullptr : ht.data(), hs.data(), N, theta, interp_degree,
-                            batch_size, leaf_size, sms);
+                            batch_size, leaf_size, sms, rank, world);
     if (rc) { delete pl; return rc; }
     pl->device = dev;
 
@@ -235,16 +250,20 @@ int bltc_create(bltc_handle* h, const double* targets, const double* sources, co
     }
     // batches, lists, work items
     {
-        const size_t nb = hp.b_begin.size();
+        // the epilogue runs over this rank's batches only (all of them unless the plan is sharded)
+        const size_t nb = (size_t)(hp.shard_b1 - hp.shard_b0);
         std::vector<int32_t> bb(nb), bc(nb), bs(nb);
-        for (size_t b = 0; b < nb; ++b) {
-            bb[b] = (int32_t)hp.b_begin[b]; bc[b] = (int32_t)(hp.b_end[b] - hp.b_begin[b]);
-            bs[b] = hp.b_nseg_far[b] + hp.b_nseg_near[b];
+        std::vector<int64_t> bp(nb);
+        for (size_t i = 0; i < nb; ++i) {
+            const size_t b = (size_t)hp.shard_b0 + i;
+            bb[i] = (int32_t)hp.b_begin[b]; bc[i] = (int32_t)(hp.b_end[b] - hp.b_begin[b]);
+            bs[i] = hp.b_nseg_far[b] + hp.b_nseg_near[b];
+            bp[i] = hp.b_partial_base[b];
         }
         BLTC_TRY_OR_FREE(pl->b_begin.upload(bb));
         BLTC_TRY_OR_FREE(pl->b_count.upload(bc));
         BLTC_TRY_OR_FREE(pl->b_nseg.upload(bs));
-        BLTC_TRY_OR_FREE(pl->b_partial_base.upload(hp.b_partial_base));
+        BLTC_TRY_OR_FREE(pl->b_partial_base.upload(bp));
         const size_t ns = hp.cluster_of_slot.size();
         std::vector<int32_t> sb(ns), se(ns);
         for (size_t s = 0; s < ns; ++s) {
@@ -310,6 +329,13 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->theta = hp.theta;
     s->build_ms = hp.build_ms;
     s->upload_ms = h->upload_ms;
+    s->shard_rank = hp.shard_rank;
+    s->shard_world = hp.shard_world;
+    s->shard_batch_begin = hp.shard_b0;
+    s->shard_batch_end = hp.shard_b1;
+    s->shard_targets = hp.shard_b1 > hp.shard_b0 ? hp.b_end[hp.shard_b1 - 1] - hp.b_begin[hp.shard_b0] : 0;
+    s->shard_far_evals = hp.shard_far_evals;
+    s->shard_near_evals = hp.shard_near_evals;
     return BLTC_OK;
 }
 
@@ -338,6 +364,16 @@ int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
     if (near_ptr) std::memcpy(near_ptr, hp.near_ptr.data(), hp.near_ptr.size() * sizeof(int64_t));
     if (far_idx) std::memcpy(far_idx, hp.far_idx.data(), hp.far_idx.size() * sizeof(int32_t));
     if (near_idx) std::memcpy(near_idx, hp.near_idx.data(), hp.near_idx.size() * sizeof(int32_t));
+    return BLTC_OK;
+}
+
+int bltc_get_shard_targets(bltc_handle h, int64_t* idx) {
+    if (!h || !idx) return fail(BLTC_EINVAL, "NULL argument");
+    const HostPlan& hp = h->hp;
+    if (hp.shard_b1 <= hp.shard_b0) return BLTC_OK;
+    const std::vector<int64_t>& perm = hp.tgt_perm();
+    const int64_t t0 = hp.b_begin[hp.shard_b0], t1 = hp.b_end[hp.shard_b1 - 1];
+    for (int64_t t = t0; t < t1; ++t) idx[t - t0] = perm[t];
     return BLTC_OK;
 }
 
@@ -378,17 +414,27 @@ int bltc_get_phase_ms(bltc_handle h, float ms[BLTC_NUM_PHASES]) {
     return BLTC_OK;
 }
 
-int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
-                  int subtract_singularity, bltc_stream stream) {
+}  // extern "C"
+
+namespace {
+
+// One convolution through the plan, kind = kYukawa (k: n_orb values) or kCoulomb (alpha; k unused).
+int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const double* f, int n_orb,
+                  double* out, int subtract_singularity, bltc_stream stream) {
     if (!h) return fail(BLTC_EINVAL, "handle is NULL");
     if (!h->on_device) return fail(BLTC_ENODEVICE, "plan was built with bltc_create_host_plan (no device state)");
-    if (!k || !f || !out) return fail(BLTC_EINVAL, "k, f and out must not be NULL");
+    if (!f || !out) return fail(BLTC_EINVAL, "f and out must not be NULL");
     if (n_orb < 1) return fail(BLTC_EINVAL, "n_orb must be >= 1");
     HostPlan& hp = h->hp;
     const bool sub = subtract_singularity != 0;
     if (sub && !hp.same_points) return fail(BLTC_EINVAL, "subtract_singularity requires targets == sources");
-    for (int o = 0; o < n_orb; ++o)
-        if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    if (kind == kYukawa) {
+        if (!k) return fail(BLTC_EINVAL, "k must not be NULL");
+        for (int o = 0; o < n_orb; ++o)
+            if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    } else if (sub && (!(alpha > 0.0) || !std::isfinite(alpha) || !(hp.max_dist / alpha < 5e5))) {
+        return fail(BLTC_EINVAL, "alpha must be finite, > 0 and > 2e-6 x the domain diameter");
+    }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int64_t N = hp.N;
 
@@ -424,11 +470,12 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
     for (size_t g = 0; g < groups.size(); ++g) {
         const int ot = groups[g];
         const int rv = targets_per_thread(ot) - 1;
-        const KPar nk = make_kpar(k + o0, ot);
+        const KPar nk = kind == kYukawa ? make_kpar(k + o0, ot) : make_kpar_coulomb(sub ? alpha : 1.0);
+        const EpiPar ep = kind == kYukawa ? make_epipar(k + o0, ot) : make_epipar_coulomb(sub ? alpha : 1.0);
         // exp underflow guard: not needed when k r < 700 for every pair (max_dist bounds r)
         double kmax = 0.0;
-        for (int o = 0; o < ot; ++o) kmax = std::max(kmax, k[o0 + o]);
-        const bool guard = !(kmax * hp.max_dist < 700.0);
+        if (kind == kYukawa) for (int o = 0; o < ot; ++o) kmax = std::max(kmax, k[o0 + o]);
+        const bool guard = kind != kYukawa || !(kmax * hp.max_dist < 700.0);
         cudaEvent_t* ev = h->profiling ? &h->events[g * per] : nullptr;
         if (ev) BLTC_CUDA(cudaEventRecord(ev[0], st));
         // a1: gather to tree order
@@ -445,17 +492,17 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
                                 h->fhat.p, h->up_chunks.p, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
         // a3: far field
-        BLTC_CUDA(launch_far(ot, sub, guard, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
+        BLTC_CUDA(launch_far(kind, ot, sub, guard, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
                              h->slot_nodes.p, h->what.p, h->fhat.p, hp.degree, h->tgt_rec, ftgt, nk,
                              h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[3], st));
         // a4: near field
-        BLTC_CUDA(launch_near(ot, sub, guard, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
+        BLTC_CUDA(launch_near(kind, ot, sub, guard, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
                               h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
         // a5: epilogue
-        BLTC_CUDA(launch_epilogue(ot, sub, (int)hp.b_begin.size(), h->b_begin.p, h->b_count.p,
-                                  h->b_partial_base.p, h->b_nseg.p, h->partial.p, hp.partial_len, ftgt, nk,
+        BLTC_CUDA(launch_epilogue(ot, sub, hp.shard_b1 - hp.shard_b0, h->b_begin.p, h->b_count.p,
+                                  h->b_partial_base.p, h->b_nseg.p, h->partial.p, hp.partial_len, ftgt, ep,
                                   h->tgt_perm, d_out, N, o0, st));
         if (ev) { BLTC_CUDA(cudaEventRecord(ev[5], st)); h->events_used += per; }
         h->last_ot = ot;
@@ -466,6 +513,20 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
         BLTC_CUDA(cudaStreamSynchronize(st));
     }
     return BLTC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
+                  int subtract_singularity, bltc_stream stream) {
+    return convolve_impl(h, kYukawa, k, 0.0, f, n_orb, out, subtract_singularity, stream);
+}
+
+int bltc_convolve_coulomb(bltc_handle h, const double* f, int n_f, double* out, int subtract_singularity,
+                          double alpha, bltc_stream stream) {
+    return convolve_impl(h, kCoulomb, nullptr, alpha, f, n_f, out, subtract_singularity, stream);
 }
 
 int bltc_direct_set_profiling(int enable) { g_direct_profiling = enable != 0; return BLTC_OK; }
@@ -483,18 +544,27 @@ int bltc_direct_get_kernel_ms(float* ms) {
     return BLTC_OK;
 }
 
-int direct_convolve(const double* targets, const double* f_targets, int64_t M,
-                    const double* sources, const double* weights, const double* f_sources, int64_t N,
-                    const double* k, int n_orb, double* out, int subtract_singularity,
-                    bltc_stream stream) {
-    if (!targets || !sources || !weights || !f_sources || !k || !out)
-        return fail(BLTC_EINVAL, "targets, sources, weights, f_sources, k and out must not be NULL");
+}  // extern "C"
+
+namespace {
+
+int direct_impl(int kind, const double* targets, const double* f_targets, int64_t M,
+                const double* sources, const double* weights, const double* f_sources, int64_t N,
+                const double* k, double alpha, int n_orb, double* out, int subtract_singularity,
+                bltc_stream stream) {
+    if (!targets || !sources || !weights || !f_sources || !out)
+        return fail(BLTC_EINVAL, "targets, sources, weights, f_sources and out must not be NULL");
     if (M < 0 || N < 0 || M > 2000000000LL || N > 2000000000LL) return fail(BLTC_EINVAL, "M, N must be in [0, 2e9]");
     if (n_orb < 1) return fail(BLTC_EINVAL, "n_orb must be >= 1");
     const bool sub = subtract_singularity != 0;
     if (sub && !f_targets) return fail(BLTC_EINVAL, "subtract_singularity needs f_targets");
-    for (int o = 0; o < n_orb; ++o)
-        if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    if (kind == kYukawa) {
+        if (!k) return fail(BLTC_EINVAL, "k must not be NULL");
+        for (int o = 0; o < n_orb; ++o)
+            if (!(k[o] > 0.0) || !std::isfinite(k[o])) return fail(BLTC_EINVAL, "every k must be finite and > 0");
+    } else if (sub && (!(alpha > 0.0) || !std::isfinite(alpha))) {
+        return fail(BLTC_EINVAL, "alpha must be finite and > 0");
+    }
     if (M == 0) return BLTC_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int dev = 0, sms = 0;
@@ -581,7 +651,8 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
         const int rv = targets_per_thread(ot) - 1;
         if (!t_items[rv].p)
             BLTC_CUDA(put(t_items[rv], items[rv].data(), items[rv].size() * sizeof(WorkItem)));
-        const KPar nk = make_kpar(k + o0, ot);
+        const KPar nk = kind == kYukawa ? make_kpar(k + o0, ot) : make_kpar_coulomb(sub ? alpha : 1.0);
+        const EpiPar ep = kind == kYukawa ? make_epipar(k + o0, ot) : make_epipar_coulomb(sub ? alpha : 1.0);
         BLTC_CUDA(launch_gather(d_fs, N, o0, ot, nullptr, N, t_fsrc.as<double>(), st));
         if (sub) BLTC_CUDA(launch_gather(d_ft, M, o0, ot, nullptr, M, t_ftgt.as<double>(), st));
         cudaEvent_t ea = nullptr, eb = nullptr;
@@ -589,13 +660,13 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
             BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
             BLTC_CUDA(cudaEventRecord(ea, st));
         }
-        BLTC_CUDA(launch_near(ot, sub, true, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
+        BLTC_CUDA(launch_near(kind, ot, sub, true, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }
         BLTC_CUDA(launch_epilogue(ot, sub, (int)npb, t_pbb.as<int32_t>(), t_pbc.as<int32_t>(),
                                   t_pbs.as<int64_t>(), t_pbn.as<int32_t>(), t_partial.as<double>(), partial_len,
-                                  t_ftgt.as<double>(), nk, nullptr, d_out, M, o0, st));
+                                  t_ftgt.as<double>(), ep, nullptr, d_out, M, o0, st));
         o0 += ot;
     }
     if (out_on_host) {
@@ -603,6 +674,25 @@ int direct_convolve(const double* targets, const double* f_targets, int64_t M,
         BLTC_CUDA(cudaStreamSynchronize(st));
     }
     return BLTC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int direct_convolve(const double* targets, const double* f_targets, int64_t M,
+                    const double* sources, const double* weights, const double* f_sources, int64_t N,
+                    const double* k, int n_orb, double* out, int subtract_singularity,
+                    bltc_stream stream) {
+    return direct_impl(kYukawa, targets, f_targets, M, sources, weights, f_sources, N, k, 0.0, n_orb, out,
+                       subtract_singularity, stream);
+}
+
+int direct_convolve_coulomb(const double* targets, const double* f_targets, int64_t M,
+                            const double* sources, const double* weights, const double* f_sources, int64_t N,
+                            int n_f, double* out, int subtract_singularity, double alpha, bltc_stream stream) {
+    return direct_impl(kCoulomb, targets, f_targets, M, sources, weights, f_sources, N, nullptr, alpha, n_f, out,
+                       subtract_singularity, stream);
 }
 
 int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream) {

@@ -241,7 +241,11 @@ template <int OT> struct SrcRec { static constexpr int kDoubles = OT <= 2 ? 6 : 
 // ZS (zero-safe): the tile may hold a source that coincides with a target -> the singular term is
 // skipped by an integer select on the rsqrt seed (reading R3).  The host flags the
 // ranges for which that can happen (bounding boxes intersect); all other tiles run the ZS = false loop.
-template <int R, int OT, bool SUB, bool GUARD, bool ZS>
+//
+// KIND = kYukawa:  acc += e^{-k_o r} (w_j / r) (f_j - f_i)                                  Eq. (20), (34)
+// KIND = kCoulomb: acc += (w_j / r) (f_j - f_i e^{-r^2/alpha^2})   (one Gaussian per pair, shared by the
+//                  orbitals of the tile; kp.c[0] = -T/(ln2 alpha^2))                        Eq. (23), (34)
+template <int R, int OT, bool SUB, bool GUARD, bool ZS, int KIND>
 __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __restrict__ tile, int j0, int j1,
                                           const KPar& kp, uint32_t tab, const MathRegs& mr) {
     constexpr int RD = SrcRec<OT>::kDoubles;
@@ -268,18 +272,27 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
             double rinv, rr;
             rsqrt_sqrt<ZS>(r2, rinv, rr, mr);              // ZS and r2 == 0: rinv = 0, the term vanishes
             const double gw = rinv * szw.y;
+            if (KIND == kCoulomb) {
+                const double gs = SUB ? exp_neg_kr<GUARD>(r2, kp.c[0], tab, mr, ec) : 0.0;   // e^{-r^2/alpha^2}
 #pragma unroll
-            for (int o = 0; o < OT; ++o) {
-                const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
-                const double g = ex * gw;
-                const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
-                T.acc[r][o] = fma(g, df, T.acc[r][o]);
+                for (int o = 0; o < OT; ++o) {
+                    const double df = SUB ? fma(-T.f[r][o], gs, sf[o]) : sf[o];   // f_j - f_i e^{-r^2/alpha^2}, Eq. (23)
+                    T.acc[r][o] = fma(gw, df, T.acc[r][o]);
+                }
+            } else {
+#pragma unroll
+                for (int o = 0; o < OT; ++o) {
+                    const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
+                    const double g = ex * gw;
+                    const double df = SUB ? (sf[o] - T.f[r][o]) : sf[o];     // (f_j - f_i), Eq. (20)
+                    T.acc[r][o] = fma(g, df, T.acc[r][o]);
+                }
             }
         }
     }
 }
 
-template <int R, int OT, bool SUB, bool GUARD>
+template <int R, int OT, bool SUB, bool GUARD, int KIND>
 __global__ void __launch_bounds__(kThreads, 2)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
@@ -320,8 +333,8 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
         }
         __syncthreads();
         const int j0 = (fill * split) >> sshift, j1 = (fill * (split + 1)) >> sshift;
-        if (flags & kRangeMayCoincide) near_tile<R, OT, SUB, GUARD, true>(T, s_tile, j0, j1, kp, tab, mr);
-        else near_tile<R, OT, SUB, GUARD, false>(T, s_tile, j0, j1, kp, tab, mr);
+        if (flags & kRangeMayCoincide) near_tile<R, OT, SUB, GUARD, true, KIND>(T, s_tile, j0, j1, kp, tab, mr);
+        else near_tile<R, OT, SUB, GUARD, false, KIND>(T, s_tile, j0, j1, kp, tab, mr);
     }
     reduce_and_store<R, OT>(T, it, warp, lane, split, 8 >> it.gshift, s_tile, partial, partial_len);
 }
@@ -333,7 +346,9 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 // next row's dx^2 + dy^2 overlaps the tail of the current one); N1 = 0: any degree.
 template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 : (OT <= 3 ? 4 : 6); };
 
-template <int R, int OT, bool SUB, bool GUARD, int N1>
+// KIND = kCoulomb: acc += (fhat_k - f_i what_k e^{-r^2/alpha^2}) / r  (reading R21: the Gaussian of Eq. (23)
+// is interpolated with the proxy weights of w).
+template <int R, int OT, bool SUB, bool GUARD, int KIND, int N1>
 __global__ void __launch_bounds__(kThreads, 2)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
@@ -415,13 +430,22 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
                         const double r2 = fma(dz, dz, dxy2[r]);
                         double rinv, rr;
                         rsqrt_sqrt<false>(r2, rinv, rr, mr);   // MAC keeps targets off the grid (theta < 1)
+                        if (KIND == kCoulomb) {
+                            const double wg = SUB ? wv * exp_neg_kr<GUARD>(r2, kp.c[0], tab, mr, ec) : 0.0;
 #pragma unroll
-                        for (int o = 0; o < OT; ++o) {
-                            const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
-                            const double g = ex * rinv;
-                            // fhat_k - f_i what_k: interpolated charges of (f_j - f_i) w_j (reading R11)
-                            const double qk = SUB ? fma(-T.f[r][o], wv, fv[o]) : fv[o];
-                            T.acc[r][o] = fma(g, qk, T.acc[r][o]);
+                            for (int o = 0; o < OT; ++o) {
+                                const double qk = SUB ? fma(-T.f[r][o], wg, fv[o]) : fv[o];
+                                T.acc[r][o] = fma(rinv, qk, T.acc[r][o]);
+                            }
+                        } else {
+#pragma unroll
+                            for (int o = 0; o < OT; ++o) {
+                                const double ex = exp_neg_kr<GUARD>(rr, kp.c[o], tab, mr, ec);
+                                const double g = ex * rinv;
+                                // fhat_k - f_i what_k: interpolated charges of (f_j - f_i) w_j (reading R11)
+                                const double qk = SUB ? fma(-T.f[r][o], wv, fv[o]) : fv[o];
+                                T.acc[r][o] = fma(g, qk, T.acc[r][o]);
+                            }
                         }
                     }
                 }
@@ -437,7 +461,7 @@ __global__ void __launch_bounds__(kThreads)
 epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__ b_count,
                 const int64_t* __restrict__ b_partial_base, const int32_t* __restrict__ b_nseg,
                 const double* __restrict__ partial, int64_t partial_len, const double* __restrict__ ftgt,
-                const KPar kp, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
+                const EpiPar ep, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
                 int o0) {
     const int b = blockIdx.x;
     const int begin = b_begin[b], count = b_count[b], nseg = b_nseg[b];
@@ -449,8 +473,8 @@ epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__
         for (int o = 0; o < OT; ++o) {
             double s = 0.0;
             for (int g = 0; g < nseg; ++g) s += partial[(int64_t)o * partial_len + base + (int64_t)g * count + l];
-            double v = -kInv2Pi * s;                               // -2 * S / (4 pi)
-            if (SUB) v = fma(-2.0 / (kp.nk[o] * kp.nk[o]), ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2
+            double v = ep.scale * s;                               // Yukawa: -2 * S / (4 pi);  Coulomb: S
+            if (SUB) v = fma(ep.coef[o], ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2 (Eq. (21)) / 2 pi alpha^2 f_i (Eq. (24))
             out[(int64_t)(o0 + o) * stride + dst] = v;
         }
     }
@@ -497,6 +521,33 @@ KPar make_kpar(const double* k, int ot) {
     kp.c1 = BLTC_EXP_C1;
     kp.c3 = BLTC_EXP_C3;
     return kp;
+}
+
+KPar make_kpar_coulomb(double alpha) {
+    KPar kp;
+    for (int o = 0; o < kMaxOT; ++o) {
+        kp.nk[o] = 0.0;
+        // e^{-r^2/alpha^2} = exp(-(1/alpha^2) r2): the same scaled-argument form as e^{-k r}
+        kp.c[o] = (double)(-(long double)BLTC_EXP_T / ((long double)alpha * (long double)alpha *
+                                                        0.693147180559945309417232121458176568L));
+    }
+    kp.c1 = BLTC_EXP_C1;
+    kp.c3 = BLTC_EXP_C3;
+    return kp;
+}
+
+EpiPar make_epipar(const double* k, int ot) {
+    EpiPar ep;
+    ep.scale = -kInv2Pi;                                   // -2 / (4 pi)
+    for (int o = 0; o < kMaxOT; ++o) ep.coef[o] = o < ot ? -2.0 / (k[o] * k[o]) : 0.0;   // Eq. (21)
+    return ep;
+}
+
+EpiPar make_epipar_coulomb(double alpha) {
+    EpiPar ep;
+    ep.scale = 1.0;
+    for (int o = 0; o < kMaxOT; ++o) ep.coef[o] = 2.0 * 3.14159265358979323846 * alpha * alpha;   // Eq. (24)
+    return ep;
 }
 
 cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
@@ -573,15 +624,26 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
 #undef BLTC_GO
 }
 
-template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD, 0>; } };
-template <int R, int OT, bool SUB, bool GUARD> struct FarK9 { static auto get() { return far_kernel<R, OT, SUB, GUARD, 9>; } };
-template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD, kYukawa, 0>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct FarK9 { static auto get() { return far_kernel<R, OT, SUB, GUARD, kYukawa, 9>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD, kYukawa>; } };
+// Coulomb: the Gaussian's exponent -r^2/alpha^2 is not bounded by a per-launch test, so the underflow guard is always on
+template <int R, int OT, bool SUB, bool GUARD> struct FarKC { static auto get() { return far_kernel<R, OT, SUB, true, kCoulomb, 0>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct FarK9C { static auto get() { return far_kernel<R, OT, SUB, true, kCoulomb, 9>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearKC { static auto get() { return near_kernel<R, OT, SUB, true, kCoulomb>; } };
 
-cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
+cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
+    if (kind == kCoulomb) {
+        if (degree == 8)
+            return dispatch_pair<FarK9C>(ot, subtract, true, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
+                                         what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
+        return dispatch_pair<FarKC>(ot, subtract, true, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
+                                    what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
+    }
     if (degree == 8)          // the paper's n = 8: grid size known at compile time
         return dispatch_pair<FarK9>(ot, subtract, guard, far_smem_bytes(ot), nitems, st, items, far_slots, slot_nodes,
                                     what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
@@ -589,18 +651,21 @@ cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items,
                                what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
 }
 
-cudaError_t launch_near(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
+cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
+    if (kind == kCoulomb)
+        return dispatch_pair<NearKC>(ot, subtract, true, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc,
+                                     tgt_rec, ftgt, kp, partial, partial_len);
     return dispatch_pair<NearK>(ot, subtract, guard, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc,
                                 tgt_rec, ftgt, kp, partial, partial_len);
 }
 
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
-                            int64_t partial_len, const double* ftgt, const KPar& kp, const int32_t* perm,
+                            int64_t partial_len, const double* ftgt, const EpiPar& kp, const int32_t* perm,
                             double* out, int64_t stride, int o0, cudaStream_t st) {
     if (nbatch == 0) return cudaSuccess;
 #define BLTC_EPI(OTV)                                                                                  \

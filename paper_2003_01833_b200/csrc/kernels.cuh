@@ -22,6 +22,16 @@ inline int targets_per_thread(int ot) { return ot <= 2 ? 2 : 1; }
 struct KPar { double nk[kMaxOT]; double c[kMaxOT]; double c1, c3; };
 KPar make_kpar(const double* k, int ot);   // k: ot values (host)
 
+// kernel of the convolution: Yukawa e^{-k r}/(4 pi r) with the subtraction of Eq. (20)-(21),
+// or Coulomb 1/r with the Gaussian subtraction of Eq. (23)-(24)
+enum { kYukawa = 0, kCoulomb = 1 };
+KPar make_kpar_coulomb(double alpha);      // c[*] = -T/(ln2 alpha^2): scaled exponent of e^{-r^2/alpha^2}
+
+// epilogue constants: out = scale * (far + near) + [subtract] coef[o] * f_i
+struct EpiPar { double scale; double coef[kMaxOT]; };
+EpiPar make_epipar(const double* k, int ot);     // scale = -2/(4 pi), coef = -2/k_o^2
+EpiPar make_epipar_coulomb(double alpha);        // scale = 1, coef = 2 pi alpha^2
+
 // a1: f[o0+o][perm[i]] -> dst[i][ot] (tree order, orbital-interleaved)
 cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const int32_t* perm,
                           int64_t n, double* dst, cudaStream_t st);
@@ -37,21 +47,22 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
                           const double* fsrc, double* out, double* chunk_out, cudaStream_t st);
 
 // a3: far field
-cudaError_t launch_far(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
+cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st);
 
 // a4 / a6: near field and brute-force direct sum (same kernel, different work items)
-cudaError_t launch_near(int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
+cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
                         const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st);
 
-// a5: out[o0+o][perm[i]] = -2 ( (far + near)/(4 pi) + [subtract] f_i / k_o^2 )
+// a5: out[o0+o][perm[i]] = ep.scale (far + near) + [subtract] ep.coef[o] f_i
+//     (Yukawa: -2 ( (far + near)/(4 pi) + f_i / k_o^2 );  Coulomb: far + near + 2 pi alpha^2 f_i)
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
-                            int64_t partial_len, const double* ftgt, const KPar& kp, const int32_t* perm,
+                            int64_t partial_len, const double* ftgt, const EpiPar& ep, const int32_t* perm,
                             double* out, int64_t stride, int o0, cudaStream_t st);
 
 // roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed

@@ -152,9 +152,30 @@ void make_tiles(int64_t tb, int64_t te, int unit, std::vector<std::pair<int32_t,
 
 }  // namespace
 
+std::vector<int> shard_cuts(const std::vector<int64_t>& batch_cost, int world) {
+    const int nb = (int)batch_cost.size();
+    long double total = 0;
+    for (int64_t c : batch_cost) total += (long double)c;
+    std::vector<int> cut(world + 1, nb);
+    cut[0] = 0;
+    long double acc = 0;
+    int r = 1;
+    for (int b = 0; b < nb && r < world; ++b) {
+        // batch b goes to the slice in which the midpoint of its cost interval falls
+        const long double mid = acc + 0.5L * (long double)batch_cost[b];
+        while (r < world && mid >= total * (long double)r / (long double)world) cut[r++] = b;
+        acc += (long double)batch_cost[b];
+    }
+    for (int i = 1; i <= world; ++i) cut[i] = std::max(cut[i], cut[i - 1]);
+    return cut;
+}
+
 void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
-                     double theta, int degree, int batch_size, int leaf_size, int sm_count) {
+                     double theta, int degree, int batch_size, int leaf_size, int sm_count,
+                     int shard_rank, int shard_world) {
     const auto t0 = std::chrono::steady_clock::now();
+    if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world)
+        throw std::invalid_argument("shard rank/world must satisfy 0 <= rank < world");
     if (!sources) throw std::invalid_argument("sources is NULL");
     if (N <= 0 || N > (int64_t)2000000000) throw std::invalid_argument("N must be in [1, 2e9]");
     if (!(theta >= 0.0) || !(theta < 1.0)) throw std::invalid_argument("theta must be in [0, 1)");
@@ -196,23 +217,39 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
 
     // line 3, decisions: per-batch interaction lists ("precomputed for each target batch")
     p.far_ptr.assign(nb + 1, 0); p.near_ptr.assign(nb + 1, 0);
+    std::vector<int64_t> b_far_evals(nb, 0), b_near_evals(nb, 0);
     for (int b = 0; b < nb; ++b) {
         p.far_ptr[b] = (int64_t)p.far_idx.size(); p.near_ptr[b] = (int64_t)p.near_idx.size();
         Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
                      p.far_idx, p.near_idx};
         tr.visit(0);
         const int64_t nt = p.b_end[b] - p.b_begin[b];
-        p.far_evals += nt * p.P * ((int64_t)p.far_idx.size() - p.far_ptr[b]);
+        b_far_evals[b] = nt * p.P * ((int64_t)p.far_idx.size() - p.far_ptr[b]);
         for (size_t q = (size_t)p.near_ptr[b]; q < p.near_idx.size(); ++q)
-            p.near_evals += nt * (p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin);
+            b_near_evals[b] += nt * (p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin);
+        p.far_evals += b_far_evals[b]; p.near_evals += b_near_evals[b];
     }
     p.far_ptr[nb] = (int64_t)p.far_idx.size(); p.near_ptr[nb] = (int64_t)p.near_idx.size();
+
+    // batch slice of this rank: equal shares of the kernel evaluations (the batches are independent given
+    // the sources and the proxy charges)
+    p.shard_rank = shard_rank; p.shard_world = shard_world;
+    {
+        std::vector<int64_t> cost(nb);
+        for (int b = 0; b < nb; ++b) cost[b] = b_far_evals[b] + b_near_evals[b];
+        const std::vector<int> cut = shard_cuts(cost, shard_world);
+        p.shard_b0 = cut[shard_rank]; p.shard_b1 = cut[shard_rank + 1];
+        for (int b = p.shard_b0; b < p.shard_b1; ++b) {
+            p.shard_far_evals += b_far_evals[b]; p.shard_near_evals += b_near_evals[b];
+        }
+    }
+    const int B0 = p.shard_b0, B1 = p.shard_b1;
 
     // proxy slots: clusters that appear in some far list (R9), with their Chebyshev grids Eq. (37)
     const int ncl = (int)p.src.cl.size();
     const int n1 = degree + 1;
     p.slot_of_cluster.assign(ncl, -1);
-    for (int32_t c : p.far_idx) p.slot_of_cluster[c] = 0;
+    for (int64_t q = p.far_ptr[B0]; q < p.far_ptr[B1]; ++q) p.slot_of_cluster[p.far_idx[q]] = 0;   // local batches' far lists
     for (int c = 0; c < ncl; ++c)
         if (p.slot_of_cluster[c] == 0) {
             p.slot_of_cluster[c] = (int32_t)p.cluster_of_slot.size();
@@ -261,7 +298,7 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
     std::vector<std::vector<Range>> merged(nb);
     std::vector<int64_t> near_src(nb, 0);
     double near_cost = 0, far_cost = 0;            // in (target group of 64) x (source) units
-    for (int b = 0; b < nb; ++b) {
+    for (int b = B0; b < B1; ++b) {
         std::vector<Range>& r = merged[b];
         for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
             const Cluster& C = p.src.cl[p.near_idx[q]];
@@ -290,7 +327,7 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
     p.b_nseg_far.assign(nb, 0); p.b_nseg_near.assign(nb, 0); p.b_partial_base.assign(nb, 0);
     std::vector<std::pair<int32_t, int32_t>> tiles; std::vector<int> gsh;
     int64_t partial = 0;
-    for (int b = 0; b < nb; ++b) {
+    for (int b = B0; b < B1; ++b) {
         const int64_t nt = p.b_end[b] - p.b_begin[b];
         // near segments: equal source counts, ranges may be cut anywhere
         std::vector<std::pair<int32_t, int32_t>> nseg_slices;    // [begin, end) into near_ranges

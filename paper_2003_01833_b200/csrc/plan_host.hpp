@@ -83,13 +83,27 @@ struct HostPlan {
     int64_t partial_len = 0;                   // doubles per orbital
     std::vector<WorkItem> far_items[2], near_items[2];   // [0]: R = 1 (32 targets/group), [1]: R = 2
 
+    // multi-GPU batch sharding: this plan carries the device work of the
+    // batches [shard_b0, shard_b1) only -- a contiguous slice of the batch list holding ~1/world of the
+    // far + near kernel evaluations.  Tree, batches and lists above are always the whole problem's.
+    int shard_rank = 0, shard_world = 1;
+    int shard_b0 = 0, shard_b1 = 0;
+    int64_t shard_far_evals = 0, shard_near_evals = 0;
+
     double max_dist = 0;                       // upper bound of |target - source| over all pairs (root boxes)
     double build_ms = 0;
 };
 
 // Throws std::invalid_argument / std::bad_alloc.  targets == nullptr: targets are the sources.
 // coords: SoA double[3][n].
+// shard_rank / shard_world: see HostPlan::shard_b0 (world = 1: the whole problem).
 void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
-                     double theta, int degree, int batch_size, int leaf_size, int sm_count);
+                     double theta, int degree, int batch_size, int leaf_size, int sm_count,
+                     int shard_rank = 0, int shard_world = 1);
+
+// Cut nb batches with the given costs into `world` contiguous slices of nearly equal cost:
+// slice r = [cut[r], cut[r+1]), cut[0] = 0, cut[world] = nb; every cut is the first batch whose
+// cost prefix reaches r/world of the total (deterministic, identical on every rank).
+std::vector<int> shard_cuts(const std::vector<int64_t>& batch_cost, int world);
 
 }  // namespace bltc

@@ -213,7 +213,7 @@ def config1(leaf_size=2000, batch_size=2000, theta=0.7, degree=8):
     eps = np.array([-3.86, -0.21])
     return Workload("cfg1_be_like", x, y, z, w, V[None, :] * psi, np.sqrt(-2.0 * eps),
                     theta, degree, leaf_size, batch_size, True,
-                    {"cells": cells[0].shape[0], "eps": eps})
+                    {"cells": cells[0].shape[0], "eps": eps, "psi": psi})
 
 
 def config2(leaf_size=2000, batch_size=2000, theta=0.7, degree=8):
@@ -227,7 +227,7 @@ def config2(leaf_size=2000, batch_size=2000, theta=0.7, degree=8):
     eps = np.sort(rng.uniform(-19.0, -0.3, size=7))
     return Workload("cfg2_co_like", x, y, z, w, V[None, :] * psi, np.sqrt(-2.0 * eps),
                     theta, degree, leaf_size, batch_size, True,
-                    {"cells": cells[0].shape[0], "eps": eps})
+                    {"cells": cells[0].shape[0], "eps": eps, "psi": psi})
 
 
 def config3(leaf_size=2000, batch_size=2000, theta=0.7, degree=8, n_orb=21):
@@ -246,7 +246,7 @@ def config3(leaf_size=2000, batch_size=2000, theta=0.7, degree=8, n_orb=21):
     eps = np.sort(rng.uniform(-10.0, -0.2, size=n_orb))
     return Workload("cfg3_c6h6_like", x, y, z, w, V[None, :] * psi, np.sqrt(-2.0 * eps),
                     theta, degree, leaf_size, batch_size, True,
-                    {"cells": cells[0].shape[0], "eps": eps})
+                    {"cells": cells[0].shape[0], "eps": eps, "psi": psi})
 
 
 def config4(N=1_000_000, k=1.0, theta=0.7, degree=8, leaf_size=2000, batch_size=2000,
@@ -277,6 +277,18 @@ def random_cloud(N, n_orb=1, seed=0, k=None, clustered=False, **kw):
     return Workload(f"cloud_N{N}_s{seed}", x, y, z, w, f, kk,
                     kw.get("theta", 0.7), kw.get("degree", 8), kw.get("leaf_size", 2000),
                     kw.get("batch_size", 2000), kw.get("subtract", True), {})
+
+
+def density_workload(c):
+    """The same mesh with ONE field: the electron density rho = 2 sum_o psi_o^2 / int psi_o^2 of the config's
+    orbitals (doubly occupied, quadrature-normalised) -- the input of the Hartree-potential convolution
+    (Eq. (19); the workload shape of PAPER.md:482-490 Table 4).  k is unused by that kernel."""
+    psi = np.atleast_2d(c.meta["psi"])
+    rho = np.zeros(c.N)
+    for o in range(psi.shape[0]):
+        rho += 2.0 * psi[o] ** 2 / float((c.w * psi[o] ** 2).sum())
+    return Workload(c.name + "_density", c.x, c.y, c.z, c.w, rho[None, :].copy(), c.k[:1].copy(),
+                    c.theta, c.degree, c.leaf_size, c.batch_size, True, dict(c.meta))
 
 
 def sample_targets(N, n, seed=0):

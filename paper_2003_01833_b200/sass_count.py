@@ -3,7 +3,7 @@
 
   python -m paper_2003_01833_b200.sass_count [--md]
 
-For every near_kernel<R,OT,SUB,GUARD> / far_kernel<R,OT,SUB,GUARD> instantiation the innermost loops that
+For every near_kernel<R,OT,SUB,GUARD,KIND> / far_kernel<R,OT,SUB,GUARD,KIND,N1> instantiation the innermost loops that
 contain MUFU.RSQ64H (one per (target, source-or-proxy) pair) are located through their backward branches
 and their opcodes are counted (near: one loop per ZS variant, ZS = the r == 0 test is compiled in).  "pair" = one target against one source / proxy point, ALL OT orbitals of the tile;
 flops = 2 DFMA + DMUL + DADD.  bench.py's FLOPS_PER_PAIR table holds the SUB = 1 rows.
@@ -52,7 +52,7 @@ def count(lib=None):
     lib = lib or _build.build()
     rows = []
     for name, ins in kernels(lib).items():
-        m = re.search(r"(near_kernel|far_kernel)ILi(\d)ELi(\d)ELb([01])ELb([01])E(?:Li(\d+)E)?", name)
+        m = re.search(r"(near_kernel|far_kernel)ILi(\d)ELi(\d)ELb([01])ELb([01])ELi(\d)E(?:Li(\d+)E)?", name)
         if not m:
             continue
         for lp in pair_loops(ins):
@@ -64,17 +64,17 @@ def count(lib=None):
             fp64 = c["DFMA"] + c["DMUL"] + c["DADD"]
             fma_pipe = sum(o in ("IMAD", "FFMA", "FMUL", "FADD") for o in ops) / pairs
             rows.append(dict(kernel=m.group(1), R=int(m.group(2)), OT=int(m.group(3)), SUB=int(m.group(4)),
-                             GUARD=int(m.group(5)), N1=int(m.group(6) or 0), ZS=zs, pairs=pairs, **c, fp64=fp64,
+                             GUARD=int(m.group(5)), KIND=int(m.group(6)), N1=int(m.group(7) or 0), ZS=zs, pairs=pairs, **c, fp64=fp64,
                              other=len(ops) / pairs - fp64, fma_pipe=fma_pipe,
                              flops=2 * c["DFMA"] + c["DMUL"] + c["DADD"]))
-    rows.sort(key=lambda r: (r["kernel"], r["R"], r["OT"], r["SUB"], r["GUARD"], r["N1"], r["ZS"]))
+    rows.sort(key=lambda r: (r["KIND"], r["kernel"], r["R"], r["OT"], r["SUB"], r["GUARD"], r["N1"], r["ZS"]))
     return rows
 
 
 def main():
     rows = count()
-    hdr = ["kernel", "R", "OT", "SUB", "GUARD", "N1", "ZS", "pairs", "DFMA", "DMUL", "DADD", "fp64", "other", "fma_pipe", "flops"]
-    names = ["kernel", "R", "OT", "SUB", "GUARD", "N1", "ZS", "pairs/iter", "DFMA/pair", "DMUL/pair", "DADD/pair", "FP64 instr/pair",
+    hdr = ["kernel", "KIND", "R", "OT", "SUB", "GUARD", "N1", "ZS", "pairs", "DFMA", "DMUL", "DADD", "fp64", "other", "fma_pipe", "flops"]
+    names = ["kernel", "KIND (0 Yukawa, 1 Coulomb)", "R", "OT", "SUB", "GUARD", "N1", "ZS", "pairs/iter", "DFMA/pair", "DMUL/pair", "DADD/pair", "FP64 instr/pair",
              "other instr/pair", "of which FMA-pipe", "flops/pair"]
     if "--md" in sys.argv:
         print("| " + " | ".join(names) + " |")

@@ -101,6 +101,8 @@ def test_bench_flops_table_matches_the_built_sass():
     seen = set()
     for r in rows:                      # every GUARD / ZS variant executes the same FP64 mix per pair
         name = "near" if r["kernel"] == "near_kernel" else ("far9" if r["N1"] == 9 else "far")
+        if r["KIND"] == 1:
+            name = "c" + name
         key = (name, r["OT"])
         assert bench.FLOPS_PER_PAIR[key] == pytest.approx(r["flops"], abs=1e-9), (key, r)
         assert r["R"] == (2 if r["OT"] <= 2 else 1)

@@ -1,0 +1,164 @@
+"""Multi-GPU batch sharding: bltc_create_sharded gives rank r of
+`world` a contiguous slice of the target batches with ~1/world of the kernel evaluations; no data-path
+collective is needed (batches are independent given the sources and the proxy charges).
+
+CPU tests: the slicing itself, and a world_size-2 `gloo` run of the whole N > 1 host logic (each rank takes its
+slice, computes it -- with the CPU oracle standing in for the device -- and the ranks assemble the result).
+GPU test: every rank's plan run one after the other on one device into one output buffer.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_2003_01833_b200 import binding as B
+from paper_2003_01833_b200 import inputs as I
+
+
+def _cloud():
+    return I.random_cloud(20000, n_orb=2, seed=21, clustered=True, leaf_size=300, batch_size=300, degree=4)
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 5, 8])
+def test_shard_slices_partition_the_batches(world):
+    c = _cloud()
+    X = c.coords()
+    full = B.bltc_get_stats(B.bltc_create_host_plan(None, X, None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size))
+    nb = full["n_batches"]
+    assert (full["shard_rank"], full["shard_world"], full["shard_batch_begin"], full["shard_batch_end"]) == (0, 1, 0, nb)
+    assert full["shard_targets"] == c.N
+    at, seen, ev = 0, [], []
+    for r in range(world):
+        p = B.bltc_create_host_plan_sharded(None, X, None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, r, world)
+        st = B.bltc_get_stats(p)
+        # the tree, batches and lists are the whole problem's on every rank
+        for key in ("n_clusters", "n_leaves", "n_batches", "n_far", "n_near", "far_evals", "near_evals"):
+            assert st[key] == full[key], key
+        assert (st["shard_rank"], st["shard_world"]) == (r, world)
+        assert st["shard_batch_begin"] == at and st["shard_batch_end"] >= at      # contiguous, in rank order
+        at = st["shard_batch_end"]
+        idx = B.bltc_get_shard_targets(p)
+        assert idx.shape[0] == st["shard_targets"]
+        e = B.bltc_export_plan(p)
+        b0, b1 = st["shard_batch_begin"], st["shard_batch_end"]
+        if b1 > b0:                                                              # exactly its batches' targets
+            np.testing.assert_array_equal(idx, e["tgt_perm"][e["b_begin"][b0]:e["b_end"][b1 - 1]])
+        seen.append(idx)
+        ev.append(st["shard_far_evals"] + st["shard_near_evals"])
+        assert st["n_proxy_clusters"] <= full["n_proxy_clusters"]
+    assert at == nb
+    allidx = np.concatenate(seen)
+    np.testing.assert_array_equal(np.sort(allidx), np.arange(c.N))               # disjoint cover of the targets
+    assert sum(ev) == full["far_evals"] + full["near_evals"]
+    # balance: no slice is further from the mean than the most expensive single batch
+    e = B.bltc_export_plan(B.bltc_create_host_plan(None, X, None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size))
+    size = e["cl_end"] - e["cl_begin"]
+    cost = np.array([(e["b_end"][b] - e["b_begin"][b]) * ((c.degree + 1) ** 3 * (e["far_ptr"][b + 1] - e["far_ptr"][b])
+                     + size[e["near_idx"][e["near_ptr"][b]:e["near_ptr"][b + 1]]].sum()) for b in range(nb)])
+    assert cost.sum() == sum(ev)
+    assert max(abs(v - cost.sum() / world) for v in ev) <= cost.max()
+
+
+def test_shard_rejects_bad_rank():
+    c = I.random_cloud(500, seed=1, leaf_size=100, batch_size=100, degree=3)
+    for rank, world in ((-1, 2), (2, 2), (0, 0)):
+        with pytest.raises(B.BltcError):
+            B.bltc_create_host_plan_sharded(None, c.coords(), None, c.N, 0.7, 3, 100, 100, rank, world)
+
+
+def test_more_ranks_than_batches_leaves_empty_slices():
+    c = I.random_cloud(300, seed=2, leaf_size=200, batch_size=200, degree=2)     # a handful of batches
+    X = c.coords()
+    nb = B.bltc_get_stats(B.bltc_create_host_plan(None, X, None, c.N, 0.7, 2, 200, 200))["n_batches"]
+    world = nb + 3
+    tot = 0
+    for r in range(world):
+        st = B.bltc_get_stats(B.bltc_create_host_plan_sharded(None, X, None, c.N, 0.7, 2, 200, 200, r, world))
+        tot += st["shard_targets"]
+    assert tot == c.N
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close()
+    return p
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    os.environ["OMP_NUM_THREADS"] = "2"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        c = I.random_cloud(6000, n_orb=2, seed=22, clustered=True, leaf_size=200, batch_size=200, degree=4)
+        p = B.bltc_create_host_plan_sharded(None, c.coords(), None, c.N, c.theta, c.degree, c.batch_size,
+                                            c.leaf_size, rank, world)
+        st = B.bltc_get_stats(p)
+        idx = B.bltc_get_shard_targets(p)
+        # the device's part, played by the CPU oracle on exactly this rank's batches (same tree: checked in
+        # test_library_host.py): out is written only for the slice's targets
+        op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+        mine = op.evaluate(c.w, c.f, c.k, batches=list(range(st["shard_batch_begin"], st["shard_batch_end"])))
+        written = ~np.isnan(mine[0])
+        assert np.array_equal(np.sort(np.nonzero(written)[0]), np.sort(idx))
+        # assembly: untouched elements are zero, so a sum over ranks is the full result (exact: x + 0)
+        out = torch.from_numpy(np.where(np.isnan(mine), 0.0, mine))
+        dist.all_reduce(out, op=dist.ReduceOp.SUM)
+        counts = torch.tensor([int(written.sum())], dtype=torch.int64)
+        dist.all_reduce(counts, op=dist.ReduceOp.SUM)
+        evals = torch.tensor([st["shard_far_evals"] + st["shard_near_evals"]], dtype=torch.int64)
+        dist.all_reduce(evals, op=dist.ReduceOp.SUM)
+        if rank == 0:
+            full = op.evaluate(c.w, c.f, c.k)
+            q.put((bool(np.array_equal(out.numpy(), full)), int(counts.item()) == c.N,
+                   int(evals.item()) == op.far_evals + op.near_evals))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_gloo_sharded_convolution_assembles_to_the_full_result(oracle_mod):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == (True, True, True), res
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kernel", ["yukawa", "coulomb"])
+def test_gpu_sharded_plans_cover_all_targets_and_match_the_oracle(oracle_mod, kernel):
+    import torch
+    assert torch.cuda.is_available()
+    c = _cloud()
+    X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+    world = 3
+    out = torch.full((c.n_orb, c.N), float("nan"), dtype=torch.float64, device="cuda")
+    seen = 0
+    for r in range(world):
+        plan = B.bltc_create_sharded(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, r, world)
+        before = torch.isnan(out[0]).sum().item()
+        if kernel == "yukawa":
+            B.bltc_convolve(plan, c.k, f, c.n_orb, out, True)
+        else:
+            B.bltc_convolve_coulomb(plan, f, c.n_orb, out, True, 0.2)
+        torch.cuda.synchronize()
+        st = B.bltc_get_stats(plan)
+        assert before - torch.isnan(out[0]).sum().item() == st["shard_targets"]   # wrote its slice, nothing else
+        seen += st["shard_targets"]
+        B.bltc_destroy(plan)
+    assert seen == c.N and not torch.isnan(out).any()
+    op = oracle_mod.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    ref = op.evaluate(c.w, c.f, c.k) if kernel == "yukawa" else op.evaluate_coulomb(c.w, c.f, alpha=0.2)
+    got = out.cpu().numpy()
+    err = max(np.linalg.norm(got[o] - ref[o]) / np.linalg.norm(ref[o]) for o in range(c.n_orb))
+    assert err <= 1e-12, err
