@@ -293,6 +293,29 @@ def run_cuda(args):
     e2e_value = jobs * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
     same = bool(np.array_equal(out_host.numpy(), out.cpu().numpy()))
 
+    # ---- NEXT-2: Green-Iteration epilogue (Alg. 2 lines 4-7) on this mesh, HBM-bound ------------------
+    gi = None
+    if rank == 0:
+        n_prev = 4
+        rng = np.random.default_rng(7)
+        phi = torch.from_numpy(rng.standard_normal((n_prev, N))).cuda()
+        psi_old = torch.from_numpy(rng.standard_normal(N)).cuda()
+        res = torch.empty(4 + n_prev, dtype=torch.float64, device="cuda")
+        gi_ms = []
+        for i in range(3 + 10):
+            psi_new = out[0].clone()
+            flush.fill_(0.0)
+            e0.record(stream)
+            B.bltc_gi_update(w, psi_old, f[0], psi_new, phi, n_prev, N, -0.5, res)
+            e1.record(stream)
+            e1.synchronize()
+            if i >= 3:
+                gi_ms.append(e0.elapsed_time(e1))
+        gi_bytes = (11 + 2 * n_prev) * 8 * N          # K1 reads 4+n, K2 reads 2+n writes 1, K3 reads 3 writes 1
+        gi_t = float(np.median(gi_ms))
+        gi = {"ms": gi_t, "n_prev": n_prev, "launches": 4, "algorithmic_bytes": gi_bytes,
+              "GBps": gi_bytes / (gi_t * 1e-3) / 1e9, "note": "L2 flushed before each call; 4 small kernels: launch-latency bound at this N"}
+
     if rank == 0:
         near_ms = phase_sum["near"] / args.steps / len(groups)      # average launch duration
         far_ms = phase_sum["far"] / args.steps / len(groups)
@@ -347,6 +370,7 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": O * N * 8,
                     "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_ms / args.steps,
                     "bitwise_equal_to_device_path": same},
+            "gi_update": gi,
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks,
             "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},

@@ -181,6 +181,27 @@ int direct_convolve_coulomb(const double* targets, const double* f_targets, int6
                             const double* sources, const double* weights, const double* f_sources, int64_t N,
                             int n_f, double* out, int subtract_singularity, double alpha, bltc_stream stream);
 
+/*
+ * the steps of Green Iteration that follow the convolution (Algorithm 2 lines 4-7,
+ * PAPER.md:127-133), fused on the device so that psi never leaves it between two convolutions:
+ *   line 4  eps_new = eps_old - <f_old, psi_old - psi_new> / <psi_new, psi_new>     (Eq. (27),
+ *           f_old = V_eff psi_old; psi_new as computed by the convolution, before lines 5-6)
+ *   line 5  psi_new <- psi_new - sum_{j < n_prev} <psi_new, phi_j> phi_j            (deflation)
+ *   line 6  psi_new <- psi_new / sqrt(<psi_new, psi_new>)
+ *   line 7  residual = sqrt(<psi_new - psi_old, psi_new - psi_old>)
+ * with <a, b> = sum_i w_i a_i b_i (reading R22: quadrature inner product; one classical Gram-Schmidt
+ * projection with coefficients taken from the un-projected psi_new, subtracted in the order j = 0, 1, ...).
+ *   w, psi_old, f_old  double[N];  psi_new double[N], IN: G(eps_old) psi_old, OUT: the new normalised iterate;
+ *   phi double[n_prev][N] orthonormal converged wavefunctions (NULL iff n_prev == 0), 0 <= n_prev <= 4096;
+ *   result double[4 + n_prev]: [0] eps_new, [1] delta = eps_old - eps_new, [2] norm before line 6,
+ *           [3] residual, [4 + j] = <psi_new, phi_j>.
+ * Every pointer may be device or host; with all pointers on the device the call only enqueues 4 kernels on
+ * `stream`; a host psi_new or result makes it synchronise.  Sums are two-level in a fixed order (reproducible).
+ */
+int bltc_gi_update(const double* w, const double* psi_old, const double* f_old, double* psi_new,
+                   const double* phi, int n_prev, int64_t N, double eps_old, double* result,
+                   bltc_stream stream);
+
 int bltc_destroy(bltc_handle h);
 
 int bltc_get_stats(bltc_handle h, bltc_stats* s);

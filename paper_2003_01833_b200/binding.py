@@ -41,7 +41,7 @@ class bltc_stats(C.Structure):
 
 EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
             "bltc_get_shard_targets", "bltc_convolve", "direct_convolve",
-            "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_destroy",
+            "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
             "bltc_probe_fp64", "bltc_last_error", "bltc_version")
@@ -69,6 +69,7 @@ def lib():
     L.bltc_convolve_coulomb.argtypes = [vp, vp, C.c_int, vp, C.c_int, C.c_double, vp]
     L.direct_convolve_coulomb.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, C.c_int, vp, C.c_int,
                                           C.c_double, vp]
+    L.bltc_gi_update.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int64, C.c_double, vp, vp]
     L.bltc_destroy.argtypes = [vp]
     L.bltc_get_stats.argtypes = [vp, C.POINTER(bltc_stats)]
     L.bltc_export_plan.argtypes = [vp, _i64p, _i64p, _i64p, _i64p, _dp, _dp, _i32p, _i32p, _i64p, _i64p,
@@ -219,6 +220,15 @@ def direct_convolve_coulomb(targets, f_targets, M, sources, weights, f_sources, 
                                          _ptr(f_sources, "f_sources"), int(N), int(n_f), _ptr(out, "out"),
                                          int(bool(subtract_singularity)), float(alpha), _stream_ptr(stream)))
     return out
+
+
+def bltc_gi_update(w, psi_old, f_old, psi_new, phi, n_prev, N, eps_old, result, stream=None):
+    """include/bltc.h bltc_gi_update (Green Iteration, Alg. 2 lines 4-7).  psi_new is updated in place;
+    result: float64[4 + n_prev] buffer (device or host) = eps_new, delta, norm, residual, coefficients."""
+    _check(lib().bltc_gi_update(_ptr(w, "w"), _ptr(psi_old, "psi_old"), _ptr(f_old, "f_old"),
+                                _ptr(psi_new, "psi_new"), _ptr(phi, "phi", True), int(n_prev), int(N),
+                                float(eps_old), _ptr(result, "result"), _stream_ptr(stream)))
+    return result
 
 
 def bltc_destroy(plan):

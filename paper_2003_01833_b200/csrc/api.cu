@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "../../include/bltc.h"
+#include "gi_kernels.cuh"
 #include "kernels.cuh"
 #include "plan_host.hpp"
 
@@ -68,7 +69,23 @@ struct TempBuf {
     ~TempBuf() { if (p) cudaFreeAsync(p, st); }
     cudaError_t alloc(size_t bytes, cudaStream_t s) {
         st = s;
+        keep_pool_memory();
         return cudaMallocAsync(&p, bytes ? bytes : 1, s);
+    }
+    // The default memory pool hands its memory back to the driver at every synchronisation unless a release
+    // threshold is set; a call that stages a few buffers would then pay a real cudaMalloc/cudaFree (~ms) each
+    // time.  Set once per device: freed blocks stay in the pool for the next call.
+    static void keep_pool_memory() {
+        static bool done[64] = {};
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || done[dev]) return;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+        done[dev] = true;
     }
     template <typename T> T* as() const { return static_cast<T*>(p); }
 };
@@ -693,6 +710,43 @@ int direct_convolve_coulomb(const double* targets, const double* f_targets, int6
                             int n_f, double* out, int subtract_singularity, double alpha, bltc_stream stream) {
     return direct_impl(kCoulomb, targets, f_targets, M, sources, weights, f_sources, N, nullptr, alpha, n_f, out,
                        subtract_singularity, stream);
+}
+
+int bltc_gi_update(const double* w, const double* psi_old, const double* f_old, double* psi_new,
+                   const double* phi, int n_prev, int64_t N, double eps_old, double* result,
+                   bltc_stream stream) {
+    if (!w || !psi_old || !f_old || !psi_new || !result) return fail(BLTC_EINVAL, "NULL argument");
+    if (N < 1 || N > 2000000000LL) return fail(BLTC_EINVAL, "N must be in [1, 2e9]");
+    if (n_prev < 0 || n_prev > 4096) return fail(BLTC_EINVAL, "n_prev must be in [0, 4096]");
+    if (n_prev > 0 && !phi) return fail(BLTC_EINVAL, "phi is NULL but n_prev > 0");
+    if (!std::isfinite(eps_old)) return fail(BLTC_EINVAL, "eps_old must be finite");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    BLTC_CUDA(cudaGetDevice(&dev));
+    BLTC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    TempBuf t_w, t_po, t_f, t_phi, t_pn, t_res, t_scratch;
+    const double *d_w, *d_po, *d_f, *d_phi;
+    BLTC_CUDA(stage_in(w, (size_t)N, t_w, st, &d_w));
+    BLTC_CUDA(stage_in(psi_old, (size_t)N, t_po, st, &d_po));
+    BLTC_CUDA(stage_in(f_old, (size_t)N, t_f, st, &d_f));
+    BLTC_CUDA(stage_in(n_prev ? phi : nullptr, (size_t)n_prev * N, t_phi, st, &d_phi));
+    const bool psi_on_host = !is_device_ptr(psi_new), res_on_host = !is_device_ptr(result);
+    double* d_pn = psi_new;
+    if (psi_on_host) {
+        BLTC_CUDA(t_pn.alloc((size_t)N * sizeof(double), st));
+        d_pn = t_pn.as<double>();
+        BLTC_CUDA(cudaMemcpyAsync(d_pn, psi_new, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
+    double* d_res = result;
+    const size_t nres = 4 + (size_t)n_prev;
+    if (res_on_host) { BLTC_CUDA(t_res.alloc(nres * sizeof(double), st)); d_res = t_res.as<double>(); }
+    const int nblk = gi_grid_blocks(N, sms);
+    BLTC_CUDA(t_scratch.alloc(gi_scratch_doubles(n_prev, nblk) * sizeof(double), st));
+    BLTC_CUDA(launch_gi_update(d_w, d_po, d_f, d_pn, d_phi, n_prev, N, eps_old, d_res, t_scratch.as<double>(), nblk, st));
+    if (psi_on_host) BLTC_CUDA(cudaMemcpyAsync(psi_new, d_pn, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (res_on_host) BLTC_CUDA(cudaMemcpyAsync(result, d_res, nres * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (psi_on_host || res_on_host) BLTC_CUDA(cudaStreamSynchronize(st));
+    return BLTC_OK;
 }
 
 int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream) {
