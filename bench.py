@@ -39,14 +39,14 @@ UNIT = "interactions/s"
 # (profiles/r01*_sass_counts.md; tests/test_library_host.py re-counts them from the built library).  flops = 2*DFMA + DMUL + DADD.
 # key: (kernel, orbital tile width OT) -> flops per (target, source/proxy point) pair for ALL OT orbitals
 FLOPS_PER_PAIR = {
-    ("near", 1): 34.0, ("near", 2): 50.0, ("near", 3): 66.0, ("near", 4): 82.0,
-    ("far", 1): 29.0, ("far", 2): 46.0, ("far", 3): 63.0, ("far", 4): 80.0,
+    ("near", 1): 32.0, ("near", 2): 46.0, ("near", 3): 60.0, ("near", 4): 74.0,
+    ("far", 1): 27.0, ("far", 2): 42.0, ("far", 3): 57.0, ("far", 4): 72.0,
     # degree 8: far_kernel<..., N1 = 9>, one (k1, k2) row of 9 proxy points per loop trip incl. its dx^2 + dy^2
-    ("far9", 1): 257.0 / 9, ("far9", 2): 410.0 / 9, ("far9", 3): 563.0 / 9, ("far9", 4): 716.0 / 9,
+    ("far9", 1): 239.0 / 9, ("far9", 2): 374.0 / 9, ("far9", 3): 509.0 / 9, ("far9", 4): 644.0 / 9,
     # Coulomb kernel with Gaussian singularity subtraction (bltc_convolve_coulomb)
-    ("cnear", 1): 33.0, ("cnear", 2): 37.0, ("cnear", 3): 41.0, ("cnear", 4): 45.0,
-    ("cfar", 1): 28.0, ("cfar", 2): 32.0, ("cfar", 3): 36.0, ("cfar", 4): 40.0,
-    ("cfar9", 1): 248.0 / 9, ("cfar9", 2): 284.0 / 9, ("cfar9", 3): 320.0 / 9, ("cfar9", 4): 356.0 / 9,
+    ("cnear", 1): 31.0, ("cnear", 2): 35.0, ("cnear", 3): 39.0, ("cnear", 4): 43.0,
+    ("cfar", 1): 26.0, ("cfar", 2): 30.0, ("cfar", 3): 34.0, ("cfar", 4): 38.0,
+    ("cfar9", 1): 230.0 / 9, ("cfar9", 2): 266.0 / 9, ("cfar9", 3): 302.0 / 9, ("cfar9", 4): 338.0 / 9,
 }
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.

@@ -33,11 +33,11 @@ constexpr double kExpMagic = 6755399441055744.0 + 1023.0 * BLTC_EXP_T;   // 1.5 
 
 __device__ const double kExpTab[BLTC_EXP_T] = {BLTC_EXP_TABLE};
 
-// Shared-memory table: the caller provides >= 2 * kExpTableBytes of dynamic shared memory at `raw`
-// (shared-window byte address); the table is placed at the next multiple of kExpTableBytes so that
-// "base | offset" addresses it.  Call with all threads, then __syncthreads().
+// Shared-memory table: the caller provides kExpTableBytes of dynamic shared memory at `raw` (shared-window byte
+// address, 16-byte aligned); entry addresses are raw + 8 j.  Call with all threads, then __syncthreads().
+constexpr int kExpTableSmemBytes = kExpTableBytes;
 __device__ __forceinline__ uint32_t exp_table_init(uint32_t raw, int tid, int nthreads) {
-    const uint32_t base = (raw + kExpTableBytes - 1) & ~(uint32_t)(kExpTableBytes - 1);
+    const uint32_t base = raw;
     for (int i = tid; i < kExpT; i += nthreads) {
         const double v = kExpTab[i];
         // entry j holds the mantissa of 2^(j/T) with the high word pre-biased by -(j << (20 - log2 T)):
@@ -100,14 +100,18 @@ __device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, c
     const double rho = fma(r, c, -nf);
     int m = __double2loint(t);
     if (GUARD) m = (__double2hiint(t) == 0x43380000) ? m : 0;
-    uint32_t r3, adr, lo, hi;
+    uint32_t r3, off, lo, hi;
     asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
-    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(adr) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8), "r"(tab));   // (a & b) | c
-    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(adr));
+    asm("and.b32 %0, %1, %2;" : "=r"(off) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8));                    // 8 j
+    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(off + tab));
     const uint32_t hi2 = hi + ((uint32_t)m << (20 - BLTC_EXP_LOG2T));       // exponent n + 1023 merged by one shift-add
     const double tj = __hiloint2double((int)hi2, (int)lo);   // 2^n * 2^(j/T)
+#if BLTC_EXP_DEG == 3
     double p = fma(rho, ec.c3, mr.c2);
     p = fma(p, rho, ec.c1);
+#else
+    const double p = fma(rho, mr.c2, ec.c1);
+#endif
     const double q = p * rho;
     return fma(tj, q, tj);                              // tj (1 + rho p(rho)); two distinct register operands
 }

@@ -303,7 +303,7 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
     static_assert(RD * kSrcTile >= R * OT * 8 * 32, "reduction scratch fits in the tile");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
-    double* s_tile = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
+    double* s_tile = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, sshift = 3 - it.gshift;
@@ -362,7 +362,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
-    double* s_pts = reinterpret_cast<double*>(smem_raw + 2 * kExpTableBytes);
+    double* s_pts = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     double* s_nodes = s_pts + kProxyTile * PD;           // [3][21]
     const MathRegs mr = math_regs_init(kMathOpaque);
     const ExpConst ec{kp.c1, kp.c3};
@@ -499,8 +499,8 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
-size_t near_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + (size_t)kSrcTile * sizeof(double) * (ot <= 2 ? 6 : 8); }
-size_t far_smem_bytes(int ot) { return 2 * (size_t)kExpTableBytes + sizeof(double) * ((size_t)kProxyTile * (ot == 1 ? 2 : (ot <= 3 ? 4 : 6)) + 3 * 21); }
+size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + (size_t)kSrcTile * sizeof(double) * (ot <= 2 ? 6 : 8); }
+size_t far_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)kProxyTile * (ot == 1 ? 2 : (ot <= 3 ? 4 : 6)) + 3 * 21); }
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {
@@ -519,7 +519,11 @@ KPar make_kpar(const double* k, int ot) {
         kp.c[o] = exp_scale_of_k(kk);
     }
     kp.c1 = BLTC_EXP_C1;
+#if BLTC_EXP_DEG == 3
     kp.c3 = BLTC_EXP_C3;
+#else
+    kp.c3 = 0.0;
+#endif
     return kp;
 }
 
@@ -532,7 +536,11 @@ KPar make_kpar_coulomb(double alpha) {
                                                         0.693147180559945309417232121458176568L));
     }
     kp.c1 = BLTC_EXP_C1;
+#if BLTC_EXP_DEG == 3
     kp.c3 = BLTC_EXP_C3;
+#else
+    kp.c3 = 0.0;
+#endif
     return kp;
 }
 
