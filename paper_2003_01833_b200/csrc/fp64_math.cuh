@@ -104,7 +104,11 @@ __device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, c
     asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
     asm("and.b32 %0, %1, %2;" : "=r"(off) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8));                    // 8 j
     asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(off + tab));
-    const uint32_t hi2 = hi + ((uint32_t)m << (20 - BLTC_EXP_LOG2T));       // exponent n + 1023 merged by one shift-add
+    // exponent n + 1023 merged by a shift and an add, both pinned to the ALU pipe: written as
+    // hi + (m << s), ptxas emits one IMAD (m * 2^s + hi) on the FMA pipe, which steals FP64-pipe issue cycles
+    uint32_t msh;
+    asm("shf.l.wrap.b32 %0, %1, %2, %3;" : "=r"(msh) : "r"(0), "r"(m), "n"(20 - BLTC_EXP_LOG2T));
+    const uint32_t hi2 = hi + msh;
     const double tj = __hiloint2double((int)hi2, (int)lo);   // 2^n * 2^(j/T)
 #if BLTC_EXP_DEG == 3
     double p = fma(rho, ec.c3, mr.c2);
