@@ -293,6 +293,37 @@ def run_cuda(args):
     e2e_value = jobs * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
     same = bool(np.array_equal(out_host.numpy(), out.cpu().numpy()))
 
+    # ---- a6: brute-force direct sum on a bounded target sample of this workload --------
+    direct = None
+    if rank == 0:
+        from paper_2003_01833_b200 import inputs as I
+        M = min(N, 16384)
+        idx = torch.from_numpy(I.sample_targets(N, M, seed=1)).cuda()
+        Tg = X[:, idx].contiguous()
+        fT = f[:, idx].contiguous()
+        dout = torch.empty((O, M), dtype=torch.float64, device="cuda")
+        B.bltc_direct_set_profiling(True)
+        d_ms, d_total = [], []
+        for i in range(2 + 5):
+            flush.fill_(0.0)
+            e0.record(stream)
+            if coulomb:
+                B.direct_convolve_coulomb(Tg, fT, M, X, w, f, N, O, dout, True, 1.0)
+            else:
+                B.direct_convolve(Tg, fT, M, X, w, f, N, c.k, O, dout, True)
+            e1.record(stream)
+            e1.synchronize()
+            if i >= 2:
+                d_ms.append(B.bltc_direct_get_kernel_ms()); d_total.append(e0.elapsed_time(e1))
+        B.bltc_direct_set_profiling(False)
+        dk = float(np.median(d_ms))
+        d_flops = sum(float(M) * N * FLOPS_PER_PAIR[(("c" if coulomb else "") + "near", g)] for g in orbital_groups(O))
+        direct = {"targets": M, "sources": N, "n_orb": O, "pair_kernel_ms": dk, "call_ms": float(np.median(d_total)),
+                  "pairs_per_s": O * float(M) * N / (dk * 1e-3), "tflops": d_flops / (dk * 1e-3) / 1e12,
+                  "frac": d_flops / (dk * 1e-3) / 1e12 / FP64_PEAK_TFLOPS_NOMINAL,
+                  "note": "direct_convolve on a seeded target sample (same pair kernel as the near field, "
+                          "r == 0 test and underflow guard compiled in)"}
+
     # ---- NEXT-2: Green-Iteration epilogue (Alg. 2 lines 4-7) on this mesh, HBM-bound ------------------
     gi = None
     if rank == 0:
@@ -370,6 +401,7 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": O * N * 8,
                     "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_ms / args.steps,
                     "bitwise_equal_to_device_path": same},
+            "direct": direct,
             "gi_update": gi,
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks,

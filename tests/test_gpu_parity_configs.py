@@ -131,3 +131,12 @@ def test_config4_random_cube(gpu, oracle_mod, k, theta, degree):
         assert e <= 1e-6
     if (theta, degree) == (0.5, 10):
         assert e <= 1e-9
+
+
+def test_config4_maximum_size_8e6(gpu, oracle_mod):
+    # BASELINE.json configs[4] at its largest N (8e6 points: 8268 batches, ~2e12 kernel evaluations, 128 MB of
+    # partial sums): the size at which int32 indexing and the work decomposition are stressed
+    c = I.config4(N=8_000_000, k=1.0, theta=0.7, degree=8)
+    e = check_full_size(gpu, oracle_mod, c, batches=[3, 8000], orbitals=[0], subtract=False,
+                        n_direct=1000, n_cpu_direct=16)
+    assert e <= 1e-6
