@@ -361,9 +361,9 @@ def run_cuda(args):
         far_tf = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
         probe = B.bltc_probe_fp64(64)
         # DRAM bytes of one near-kernel launch of THIS workload from the committed ncu capture
-        # (profiles/r01c_near_kernel_ncu.md names the command); null for other workloads / kernels
+        # (profiles/r01g_summary.md names the command); null for other workloads / kernels
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r01c_near_cfg1_dram.csv")
+        tpath = os.path.join(ROOT, "profiles", "r01g_near_cfg1_dram.csv")
         if args.workload == "cfg1" and not coulomb and os.path.exists(tpath):
             try:
                 import csv
