@@ -13,7 +13,7 @@
 // through shared memory in a fixed order and written to a per-(batch, segment) slice of the
 // partial buffer; the epilogue adds the slices in a fixed order => bitwise reproducible results.
 //
-// The bound is the FP64 pipe ("Roofline"): ~27 (near) / ~22 (far) FP64 instructions
+// The bound is the FP64 pipe ("Roofline"): 22 (near) / 16.4 (far, n = 8) FP64 instructions
 // per kernel evaluation for one orbital; everything else (LDS, MUFU seed, integer exponent work,
 // loop control) issues in the shadow of the half-rate FP64 pipe.
 #include "kernels.cuh"
