@@ -12,7 +12,7 @@ SOURCES = ["api.cu", "kernels.cu", "gi_kernels.cu", "plan_host.cpp"]
 HEADERS = ["kernels.cuh", "gi_kernels.cuh", "fp64_math.cuh", "plan_host.hpp", os.path.join("..", "..", "include", "bltc.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall",
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall,-pthread",
     "-shared",
 ]
 

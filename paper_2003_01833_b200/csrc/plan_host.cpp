@@ -6,8 +6,10 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <future>
 #include <numeric>
 #include <stdexcept>
+#include <thread>
 
 namespace bltc {
 namespace {
@@ -15,53 +17,59 @@ namespace {
 constexpr double kSqrt2 = 1.4142135623730951;
 constexpr double kPi = 3.14159265358979323846;
 
+// Sub-trees of different children touch disjoint ranges of perm / tmp / code, so the children of the top
+// kParLevels levels are built by concurrent tasks into private cluster vectors (local ids, DFS pre-order) and
+// spliced behind their parent in child order: the result is identical to the sequential build, cluster for
+// cluster (stage 1 "scales worst ... due to some serial computation").
 struct TreeBuilder {
+    static constexpr int kParLevels = 2;                 // up to 64 concurrent sub-tree tasks
+    static constexpr int64_t kParMin = 100000;           // smaller clusters are not worth a thread
     const double* c[3];
     int64_t max_leaf;
-    Tree& t;
+    std::vector<int64_t>& perm;
     std::vector<int64_t> tmp;
     std::vector<uint8_t> code;
 
-    TreeBuilder(Tree& tree, const double* x, const double* y, const double* z, int64_t n, int64_t ml)
-        : c{x, y, z}, max_leaf(ml), t(tree), tmp(n), code(n) {
-        t.perm.resize(n);
-        std::iota(t.perm.begin(), t.perm.end(), int64_t(0));
+    TreeBuilder(std::vector<int64_t>& perm_, const double* x, const double* y, const double* z, int64_t n, int64_t ml)
+        : c{x, y, z}, max_leaf(ml), perm(perm_), tmp(n), code(n) {
+        perm.resize(n);
+        std::iota(perm.begin(), perm.end(), int64_t(0));
     }
 
-    // bisection at the box midpoint, children shrunk to their particles.
-    int subdivide(int64_t b, int64_t e, int parent, int level) {
-        const int id = (int)t.cl.size();
-        t.cl.emplace_back();
-        {
-            Cluster& C = t.cl.back();
-            C.begin = b; C.end = e; C.parent = parent; C.level = level;
-            for (int d = 0; d < 3; ++d) {
-                double lo = c[d][t.perm[b]], hi = lo;
-                for (int64_t i = b + 1; i < e; ++i) {
-                    const double v = c[d][t.perm[i]];
-                    lo = v < lo ? v : lo;
-                    hi = v > hi ? v : hi;
-                }
-                C.lo[d] = lo; C.hi[d] = hi;
+    // Appends the cluster of [b, e) to `out` and returns its id; fills count/first with the split (all counts 0:
+    // the cluster is a leaf).  PAPER.md:378: bisection at the box midpoint, children shrunk to their particles.
+    int make_cluster(int64_t b, int64_t e, int parent, int level, std::vector<Cluster>& out, int64_t count[8],
+                     int64_t first[8]) {
+        const int id = (int)out.size();
+        out.emplace_back();
+        Cluster& C = out.back();
+        C.begin = b; C.end = e; C.parent = parent; C.level = level;
+        for (int d = 0; d < 3; ++d) {
+            double lo = c[d][perm[b]], hi = lo;
+            for (int64_t i = b + 1; i < e; ++i) {
+                const double v = c[d][perm[i]];
+                lo = v < lo ? v : lo;
+                hi = v > hi ? v : hi;
             }
+            C.lo[d] = lo; C.hi[d] = hi;
         }
+        for (int q = 0; q < 8; ++q) count[q] = 0;
         if (e - b <= max_leaf) return id;                         // R4: leaf iff count <= N_L
         double ext[3], longest = 0.0, mid[3];
         bool cut[3];
         int ncut = 0;
         for (int d = 0; d < 3; ++d) {
-            ext[d] = t.cl[id].hi[d] - t.cl[id].lo[d];
+            ext[d] = C.hi[d] - C.lo[d];
             longest = ext[d] > longest ? ext[d] : longest;
         }
         for (int d = 0; d < 3; ++d) {                             // R5: aspect-ratio rule sqrt(2)
             cut[d] = ext[d] > 0.0 && ext[d] * kSqrt2 >= longest;
             ncut += cut[d];
-            mid[d] = 0.5 * (t.cl[id].lo[d] + t.cl[id].hi[d]);
+            mid[d] = 0.5 * (C.lo[d] + C.hi[d]);
         }
         if (ncut == 0) return id;                                 // all particles coincide
-        int64_t count[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         for (int64_t i = b; i < e; ++i) {
-            const int64_t p = t.perm[i];
+            const int64_t p = perm[i];
             uint8_t k = 0;
             if (cut[0] && c[0][p] > mid[0]) k |= 1;               // bit0 x, bit1 y, bit2 z
             if (cut[1] && c[1][p] > mid[1]) k |= 2;
@@ -71,16 +79,48 @@ struct TreeBuilder {
         }
         int live = 0;
         for (int q = 0; q < 8; ++q) live += count[q] != 0;
-        if (live < 2) return id;                                  // midpoint rounded onto a face
-        int64_t first[8], cur[8];
+        if (live < 2) {                                           // midpoint rounded onto a face
+            for (int q = 0; q < 8; ++q) count[q] = 0;
+            return id;
+        }
+        int64_t cur[8];
         int64_t at = b;
         for (int q = 0; q < 8; ++q) { first[q] = cur[q] = at; at += count[q]; }
-        for (int64_t i = b; i < e; ++i) tmp[cur[code[i]]++] = t.perm[i];   // stable
-        std::copy(tmp.begin() + b, tmp.begin() + e, t.perm.begin() + b);
+        for (int64_t i = b; i < e; ++i) tmp[cur[code[i]]++] = perm[i];     // stable
+        std::copy(tmp.begin() + b, tmp.begin() + e, perm.begin() + b);
+        return id;
+    }
+
+    int subdivide(int64_t b, int64_t e, int parent, int level, int par_levels, std::vector<Cluster>& out) {
+        int64_t count[8], first[8];
+        const int id = make_cluster(b, e, parent, level, out, count, first);
+        if (par_levels > 0 && e - b >= kParMin) {
+            std::vector<Cluster> frag[8];
+            std::vector<std::future<void>> tasks;
+            for (int q = 0; q < 8; ++q) {
+                if (!count[q]) continue;                          // empty children dropped
+                tasks.push_back(std::async(std::launch::async, [this, &frag, q, &first, &count, level, par_levels] {
+                    subdivide(first[q], first[q] + count[q], -1, level + 1, par_levels - 1, frag[q]);
+                }));
+            }
+            for (auto& t : tasks) t.get();
+            for (int q = 0; q < 8; ++q) {
+                if (!count[q]) continue;
+                const int base = (int)out.size();
+                for (Cluster C : frag[q]) {
+                    C.parent = C.parent < 0 ? id : C.parent + base;
+                    for (int k = 0; k < C.nchild; ++k) C.child[k] += base;
+                    out.push_back(C);
+                }
+                Cluster& P = out[id];
+                P.child[P.nchild++] = base;
+            }
+            return id;
+        }
         for (int q = 0; q < 8; ++q) {
             if (!count[q]) continue;                              // empty children dropped
-            const int ch = subdivide(first[q], first[q] + count[q], id, level + 1);
-            Cluster& C = t.cl[id];
+            const int ch = subdivide(first[q], first[q] + count[q], id, level + 1, 0, out);
+            Cluster& C = out[id];
             C.child[C.nchild++] = ch;
         }
         return id;
@@ -94,8 +134,8 @@ void gather_leaves(const Tree& t, int id, std::vector<int>& out) {
 
 void build_tree(Tree& t, const double* x, const double* y, const double* z, int64_t n, int64_t max_leaf) {
     t.cl.clear();
-    TreeBuilder tb(t, x, y, z, n, max_leaf);
-    tb.subdivide(0, n, -1, 0);
+    TreeBuilder tb(t.perm, x, y, z, n, max_leaf);
+    tb.subdivide(0, n, -1, 0, TreeBuilder::kParLevels, t.cl);
     t.leaves.clear();
     gather_leaves(t, 0, t.leaves);
 }
@@ -215,21 +255,46 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         for (int d = 0; d < 3; ++d) { p.b_lo[3 * b + d] = L.lo[d]; p.b_hi[3 * b + d] = L.hi[d]; }
     }
 
-    // line 3, decisions: per-batch interaction lists ("precomputed for each target batch")
+    // line 3, decisions: per-batch interaction lists ("precomputed for each target batch").
+    // Batches are independent: contiguous chunks of them are traversed by concurrent tasks into private
+    // lists, concatenated in batch order (identical to the sequential result).
     p.far_ptr.assign(nb + 1, 0); p.near_ptr.assign(nb + 1, 0);
     std::vector<int64_t> b_far_evals(nb, 0), b_near_evals(nb, 0);
-    for (int b = 0; b < nb; ++b) {
-        p.far_ptr[b] = (int64_t)p.far_idx.size(); p.near_ptr[b] = (int64_t)p.near_idx.size();
-        Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
-                     p.far_idx, p.near_idx};
-        tr.visit(0);
-        const int64_t nt = p.b_end[b] - p.b_begin[b];
-        b_far_evals[b] = nt * p.P * ((int64_t)p.far_idx.size() - p.far_ptr[b]);
-        for (size_t q = (size_t)p.near_ptr[b]; q < p.near_idx.size(); ++q)
-            b_near_evals[b] += nt * (p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin);
-        p.far_evals += b_far_evals[b]; p.near_evals += b_near_evals[b];
+    {
+        const int hw = (int)std::max(1u, std::thread::hardware_concurrency());
+        const int nchunk = std::max(1, std::min(hw, nb / 64));
+        std::vector<std::vector<int32_t>> cfar(nchunk), cnear(nchunk);
+        std::vector<int64_t> nfar(nb, 0), nnear(nb, 0);
+        auto work = [&](int ch) {
+            const int b0 = (int)((int64_t)nb * ch / nchunk), b1 = (int)((int64_t)nb * (ch + 1) / nchunk);
+            for (int b = b0; b < b1; ++b) {
+                const size_t f0 = cfar[ch].size(), n0 = cnear[ch].size();
+                Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
+                             cfar[ch], cnear[ch]};
+                tr.visit(0);
+                nfar[b] = (int64_t)(cfar[ch].size() - f0); nnear[b] = (int64_t)(cnear[ch].size() - n0);
+                const int64_t nt = p.b_end[b] - p.b_begin[b];
+                b_far_evals[b] = nt * p.P * nfar[b];
+                for (size_t q = n0; q < cnear[ch].size(); ++q)
+                    b_near_evals[b] += nt * (p.src.cl[cnear[ch][q]].end - p.src.cl[cnear[ch][q]].begin);
+            }
+        };
+        if (nchunk == 1) work(0);
+        else {
+            std::vector<std::future<void>> tasks;
+            for (int ch = 0; ch < nchunk; ++ch) tasks.push_back(std::async(std::launch::async, work, ch));
+            for (auto& t : tasks) t.get();
+        }
+        for (int b = 0; b < nb; ++b) {
+            p.far_ptr[b + 1] = p.far_ptr[b] + nfar[b]; p.near_ptr[b + 1] = p.near_ptr[b] + nnear[b];
+            p.far_evals += b_far_evals[b]; p.near_evals += b_near_evals[b];
+        }
+        p.far_idx.reserve((size_t)p.far_ptr[nb]); p.near_idx.reserve((size_t)p.near_ptr[nb]);
+        for (int ch = 0; ch < nchunk; ++ch) {
+            p.far_idx.insert(p.far_idx.end(), cfar[ch].begin(), cfar[ch].end());
+            p.near_idx.insert(p.near_idx.end(), cnear[ch].begin(), cnear[ch].end());
+        }
     }
-    p.far_ptr[nb] = (int64_t)p.far_idx.size(); p.near_ptr[nb] = (int64_t)p.near_idx.size();
 
     // batch slice of this rank: equal shares of the kernel evaluations (the batches are independent given
     // the sources and the proxy charges)
