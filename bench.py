@@ -112,7 +112,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload(name="cfg1", kernel="yukawa"):
+def workload(name="cfg1", kernel="yukawa", orbitals=0):
     """cfg1 (BASELINE.json configs[1]) is the bench workload; the others are for profiling and context runs.
     kernel = "coulomb": the same mesh with ONE field, the density rho = 2 sum_o psi_o^2 -- the Hartree
     potential of bltc_convolve_coulomb (Table 4's workload shape)."""
@@ -120,6 +120,11 @@ def workload(name="cfg1", kernel="yukawa"):
     c = {"cfg0": I.config0, "cfg1": I.config1, "cfg2": I.config2, "cfg3": I.config3}[name]()
     if kernel == "coulomb":
         c = I.density_workload(c)
+    if orbitals > 0:      # profiling aid: the config's fields cycled to `orbitals` orbitals, k spread by 7 % steps
+        src = c.f.copy(); k0 = c.k.copy()
+        c.f = np.ascontiguousarray(np.stack([src[o % src.shape[0]] * (1.0 + 0.01 * o) for o in range(orbitals)]))
+        c.k = np.array([k0[o % k0.shape[0]] * (1.0 + 0.07 * (o // k0.shape[0])) for o in range(orbitals)])
+        c.name += f"_x{orbitals}orb"
     return c
 
 
@@ -168,7 +173,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    c = workload(args.workload, args.kernel)
+    c = workload(args.workload, args.kernel, args.orbitals)
     batches = [137] if args.workload == "cfg1" else 1
     vals = []
     for i in range(args.warmup + args.steps):
@@ -207,7 +212,7 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
 
-    c = workload(args.workload, args.kernel)
+    c = workload(args.workload, args.kernel, args.orbitals)
     coulomb = args.kernel == "coulomb"
     N, O = c.N, c.n_orb
 
@@ -425,6 +430,8 @@ def main():
                          "batches = one convolution, target batches sharded over the ranks (strong scaling)")
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"],
                     help="cfg1 = BASELINE.json configs[1] (the bench line); others: profiling / context")
+    ap.add_argument("--orbitals", type=int, default=0,
+                    help="profiling aid: cycle the workload's fields to this many orbitals (0 = as configured)")
     ap.add_argument("--kernel", default="yukawa", choices=["yukawa", "coulomb"],
                     help="coulomb: Hartree potential with Gaussian singularity subtraction (NEXT-1)")
     args = ap.parse_args()
