@@ -79,6 +79,21 @@ def test_more_ranks_than_batches_leaves_empty_slices():
     assert tot == c.N
 
 
+def test_shards_with_separate_targets_and_second_tree():
+    # targets != sources (batches from a second tree) and N_B != N_L: slices are cut over the TARGET batches
+    c = I.random_cloud(8000, seed=23, leaf_size=300, batch_size=120, degree=3)
+    rng = np.random.default_rng(5)
+    T = np.ascontiguousarray(rng.random((3, c.N)))
+    world, seen = 4, []
+    for r in range(world):
+        p = B.bltc_create_host_plan_sharded(T, c.coords(), None, c.N, 0.7, 3, 120, 300, r, world)
+        st = B.bltc_get_stats(p)
+        assert st["shared_batches"] == 0
+        seen.append(B.bltc_get_shard_targets(p))
+        assert len(seen[-1]) == st["shard_targets"]
+    np.testing.assert_array_equal(np.sort(np.concatenate(seen)), np.arange(c.N))
+
+
 def _free_port():
     s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close()
     return p
