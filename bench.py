@@ -221,6 +221,8 @@ def run_cuda(args):
             B.bltc_convolve_coulomb(plan, f_, O, out_, True, 1.0)
         else:
             B.bltc_convolve(plan, c.k, f_, O, out_, True)
+        if exchange is not None and out_.is_cuda:
+            exchange.all_gather_out(out_)
 
     X = torch.from_numpy(c.coords()).cuda()
     w = torch.from_numpy(c.w).cuda()
@@ -228,8 +230,12 @@ def run_cuda(args):
     out = torch.zeros((O, N), dtype=torch.float64, device="cuda")      # a sharded plan writes its slice only
     t0 = time.perf_counter()
     sharded = args.shard == "batches" and world > 1
-    if sharded:      # strong scaling: rank r computes its slice of the target batches, no collective
+    exchange = None
+    if sharded:      # strong scaling: rank r computes its slice of the target batches; the only exchange is the
+        # all-gather of `out` that the next Green-Iteration step needs on every rank
+        from paper_2003_01833_b200.multi_gpu import ShardExchange
         plan = B.bltc_create_sharded(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
+        exchange = ShardExchange(B.bltc_get_shard_targets(plan), N, "cuda")
     else:
         plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
     create_ms = (time.perf_counter() - t0) * 1e3
@@ -387,7 +393,7 @@ def run_cuda(args):
                        "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
                        "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
                        "parallelism": ("1 GPU" if world == 1 else
-                                       f"target batches sharded over {world} ranks, no collective" if sharded
+                                       f"target batches sharded over {world} ranks + all-gather of out (NCCL)" if sharded
                                        else f"{world} replicas (each rank its own orbitals), no collective")},
             "time_per_convolution_ms": ms_per_step / O,
             "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * world / (ms_per_step * 1e-3),

@@ -1,0 +1,83 @@
+"""Batch-sharded convolution over several ranks.
+
+One process per GPU.  Every rank builds the same tree and lists and owns a contiguous slice of the target batches
+(`bltc_create_sharded`); the convolution itself needs no communication.  What does need one exchange is the NEXT
+Green-Iteration step: its source field f = V_eff * psi_new is needed at ALL points on every rank (the sources are
+replicated), so after the convolution the ranks all-gather their slices of `out` -- O * N * 8 bytes in total per
+step, over NCCL (NVLink 5 / NVSwitch) for CUDA tensors, or gloo for CPU tensors (tests).
+
+This module is plumbing only (torch.distributed + index bookkeeping); all arithmetic stays in the CUDA kernels.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import binding as B
+
+
+class ShardExchange:
+    """All-gather of per-rank slices of out[n_orb][N] given each rank's target indices (caller order).
+
+    Built once per plan: the index lists of all ranks are exchanged here, so a step moves values only.
+    """
+
+    def __init__(self, shard_idx, N, device, group=None):
+        import torch
+        import torch.distributed as dist
+        self.dist, self.torch, self.group = dist, torch, group
+        self.world = dist.get_world_size(group)
+        self.rank = dist.get_rank(group)
+        self.N = int(N)
+        idx = torch.as_tensor(np.ascontiguousarray(shard_idx), dtype=torch.int64, device=device)
+        counts = torch.zeros(self.world, dtype=torch.int64, device=device)
+        counts[self.rank] = idx.numel()
+        dist.all_reduce(counts, op=dist.ReduceOp.SUM, group=group)
+        self.counts = [int(v) for v in counts.cpu()]
+        if sum(self.counts) != self.N:
+            raise ValueError(f"shards cover {sum(self.counts)} of {self.N} targets")
+        self.cmax = max(self.counts)
+        pad = torch.zeros(self.cmax, dtype=torch.int64, device=device)
+        pad[: idx.numel()] = idx
+        gathered = [torch.empty_like(pad) for _ in range(self.world)]
+        dist.all_gather(gathered, pad, group=group)
+        self.idx = [g[: self.counts[r]] for r, g in enumerate(gathered)]      # every rank's targets
+        allidx = torch.cat(self.idx)
+        if int(torch.unique(allidx).numel()) != self.N:
+            raise ValueError("shards overlap")
+        self.local_idx = idx
+
+    def all_gather_out(self, out):
+        """out: [n_orb][N] tensor whose columns `local_idx` are valid on this rank; on return every column is."""
+        torch, dist = self.torch, self.dist
+        n_orb = out.shape[0]
+        send = torch.zeros((n_orb, self.cmax), dtype=out.dtype, device=out.device)
+        send[:, : self.counts[self.rank]] = out[:, self.local_idx]
+        recv = [torch.empty_like(send) for _ in range(self.world)]
+        dist.all_gather(recv, send, group=self.group)
+        for r in range(self.world):
+            if r != self.rank and self.counts[r]:
+                out[:, self.idx[r]] = recv[r][:, : self.counts[r]]
+        return out
+
+
+class ShardedPlan:
+    """bltc_create_sharded + the exchange: `convolve` leaves the full out[n_orb][N] on every rank."""
+
+    def __init__(self, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, group=None):
+        import torch.distributed as dist
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.plan = B.bltc_create_sharded(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size,
+                                          self.rank, self.world)
+        self.stats = B.bltc_get_stats(self.plan)
+        self.exchange = ShardExchange(B.bltc_get_shard_targets(self.plan), N, sources.device, group)
+
+    def convolve(self, k, f, n_orb, out, subtract_singularity=True, gather=True):
+        B.bltc_convolve(self.plan, k, f, n_orb, out, subtract_singularity)
+        return self.exchange.all_gather_out(out) if gather else out
+
+    def convolve_coulomb(self, f, n_f, out, subtract_singularity=True, alpha=1.0, gather=True):
+        B.bltc_convolve_coulomb(self.plan, f, n_f, out, subtract_singularity, alpha)
+        return self.exchange.all_gather_out(out) if gather else out
+
+    def destroy(self):
+        B.bltc_destroy(self.plan)

@@ -118,9 +118,17 @@ def _gloo_worker(rank, world, port, q):
         mine = op.evaluate(c.w, c.f, c.k, batches=list(range(st["shard_batch_begin"], st["shard_batch_end"])))
         written = ~np.isnan(mine[0])
         assert np.array_equal(np.sort(np.nonzero(written)[0]), np.sort(idx))
-        # assembly: untouched elements are zero, so a sum over ranks is the full result (exact: x + 0)
-        out = torch.from_numpy(np.where(np.isnan(mine), 0.0, mine))
-        dist.all_reduce(out, op=dist.ReduceOp.SUM)
+        # assembly, the product's way: ShardExchange all-gathers the slices (values only; indices exchanged once)
+        from paper_2003_01833_b200.multi_gpu import ShardExchange
+        ex = ShardExchange(idx, c.N, "cpu")
+        assert ex.counts[rank] == len(idx) and sum(ex.counts) == c.N
+        out = torch.from_numpy(mine.copy())                       # NaN outside this rank's slice
+        ex.all_gather_out(out)
+        assert not torch.isnan(out).any()
+        # and the simple way: untouched elements zero, sum over ranks (exact: x + 0) -- must agree bitwise
+        out2 = torch.from_numpy(np.where(np.isnan(mine), 0.0, mine))
+        dist.all_reduce(out2, op=dist.ReduceOp.SUM)
+        assert torch.equal(out, out2)
         counts = torch.tensor([int(written.sum())], dtype=torch.int64)
         dist.all_reduce(counts, op=dist.ReduceOp.SUM)
         evals = torch.tensor([st["shard_far_evals"] + st["shard_near_evals"]], dtype=torch.int64)
@@ -177,3 +185,28 @@ def test_gpu_sharded_plans_cover_all_targets_and_match_the_oracle(oracle_mod, ke
     got = out.cpu().numpy()
     err = max(np.linalg.norm(got[o] - ref[o]) / np.linalg.norm(ref[o]) for o in range(c.n_orb))
     assert err <= 1e-12, err
+
+
+@pytest.mark.gpu
+def test_gpu_sharded_plan_with_nccl_world1_equals_plain_convolve():
+    # the CUDA-tensor path of ShardedPlan / ShardExchange (NCCL backend; a 1-rank group is all one GPU allows)
+    import torch
+    import torch.distributed as dist
+    from paper_2003_01833_b200.multi_gpu import ShardedPlan
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(_free_port())
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        c = I.random_cloud(6000, n_orb=3, seed=24, clustered=True, leaf_size=200, batch_size=200, degree=4)
+        X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+        f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+        sp = ShardedPlan(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+        out = torch.full((c.n_orb, c.N), float("nan"), dtype=torch.float64, device="cuda")
+        sp.convolve(c.k, f, c.n_orb, out)
+        plan = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+        ref = torch.empty_like(out)
+        B.bltc_convolve(plan, c.k, f, c.n_orb, ref)
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref)
+        sp.destroy(); B.bltc_destroy(plan)
+    finally:
+        dist.destroy_process_group()
