@@ -181,3 +181,24 @@ def test_coulomb_rejects_bad_arguments(gpu):
     B.bltc_convolve_coulomb(plan, f, 1, out, False, 0.0)               # alpha ignored without subtraction
     torch.cuda.synchronize()
     B.bltc_destroy(plan)
+
+
+def test_coulomb_bltc_hydrogen_hartree_potential_and_energy_closed_form(gpu):
+    # physical pin of the whole GPU path without the oracle: rho = e^{-2r}/pi on the adaptive mesh, all 387,584 targets:
+    # V_H = 1/r - e^{-2r}(1 + 1/r) and E_H = 1/2 int rho V_H = 5/16 Ha (textbook)
+    torch, B = gpu
+    h = I.hydrogen_adaptive()
+    X = dev(torch, h.coords()); w = dev(torch, h.w)
+    r = torch.sqrt((X ** 2).sum(0))
+    rho = (torch.exp(-2 * r) / np.pi).reshape(1, h.N).contiguous()
+    plan = B.bltc_create(None, X, w, h.N, 0.7, 8, 2000, 2000)
+    out = torch.empty((1, h.N), dtype=torch.float64, device="cuda")
+    B.bltc_convolve_coulomb(plan, rho, 1, out, True, 1.0)
+    torch.cuda.synchronize()
+    B.bltc_destroy(plan)
+    exact = 1 / r - torch.exp(-2 * r) * (1 + 1 / r)
+    err_w = float(torch.sqrt((w * (out[0] - exact) ** 2).sum() / (w * exact ** 2).sum()))
+    e_h = float(0.5 * (w * rho[0] * out[0]).sum())
+    print(f"hydrogen Hartree on GPU: V_H weighted L2 error {err_w:.2e}, E_H = {e_h:.7f} (5/16 = 0.3125)")
+    assert err_w < 1e-4                                  # measured: 8.7e-6
+    assert abs(e_h - 0.3125) < 2e-5                     # measured: 0.3125039
