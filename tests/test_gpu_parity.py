@@ -265,3 +265,48 @@ def test_fp64_probe_runs(gpu):
     torch, B = gpu
     t = B.bltc_probe_fp64(16)
     assert 5.0 < t < 80.0, t
+
+
+def test_bltc_fuzz_degenerate_shapes(gpu, oracle_mod):
+    # seeded sweep over odd sizes and shapes: tiny N, leaf size 1-2, planar / collinear clouds (degenerate boxes, R8),
+    # every point duplicated (r == 0 pairs between different indices, R3); Yukawa and Coulomb, subtraction on / off
+    torch, B = gpu
+    rng = np.random.default_rng(20030183 + 78)
+    worst = 0.0
+    for case in range(24):
+        N = int(rng.choice([2, 3, 17, 64, 257, 1000, 2500]))
+        leaf = int(rng.choice([1, 2, 7, 32, 100, 300]))
+        theta = float(rng.choice([0.0, 0.5, 0.8, 0.95]))
+        degree = int(rng.integers(1, 7))
+        n_orb = int(rng.integers(1, 6))
+        X = rng.random((3, N))
+        shape = case % 4
+        if shape == 1:
+            X[2] = 0.25
+        elif shape == 2:
+            X[1] = X[0]; X[2] = 0.5
+        elif shape == 3 and N > 3:
+            X[:, N // 2:] = X[:, : N - N // 2]
+        X = np.ascontiguousarray(X)
+        w = rng.random(N) / N
+        f = rng.uniform(-1, 1, (n_orb, N))
+        k = rng.uniform(0.5, 5.0, n_orb)
+        subtract = bool(case % 2)
+        op = oracle_mod.OraclePlan((X[0], X[1], X[2]), theta, degree, leaf, leaf)
+        plan = B.bltc_create(None, dev(torch, X), dev(torch, w), N, theta, degree, leaf, leaf)
+        out = torch.empty((n_orb, N), dtype=torch.float64, device="cuda")
+        B.bltc_convolve(plan, k, dev(torch, f), n_orb, out, subtract)
+        cout = torch.empty_like(out)
+        B.bltc_convolve_coulomb(plan, dev(torch, f), n_orb, cout, subtract, 0.3)
+        torch.cuda.synchronize()
+        B.bltc_destroy(plan)
+        ref = op.evaluate(w, f, k, subtract=subtract)
+        cref = op.evaluate_coulomb(w, f, subtract=subtract, alpha=0.3)
+        for got, want, what in ((out.cpu().numpy(), ref, "yukawa"), (cout.cpu().numpy(), cref, "coulomb")):
+            assert np.all(np.isfinite(got)), (case, what)
+            scale = np.linalg.norm(want, axis=1)
+            err = np.linalg.norm(got - want, axis=1)
+            ok = (err <= TOL_BLTC * np.maximum(scale, 1e-300)) | (err <= 1e-300)
+            assert ok.all(), (case, what, N, leaf, theta, degree, subtract, err, scale)
+            worst = max(worst, float((err / np.maximum(scale, 1e-300)).max()))
+    print(f"fuzz: worst relative error {worst:.2e}")

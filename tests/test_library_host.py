@@ -57,6 +57,11 @@ CASES = [
     ("ragged", lambda: I.random_cloud(7777, seed=11, leaf_size=333, batch_size=333, degree=3, theta=0.5)),
     ("one_leaf", lambda: I.random_cloud(500, seed=12, leaf_size=2000, batch_size=2000)),
     ("theta0", lambda: I.random_cloud(2000, seed=13, leaf_size=100, batch_size=100, theta=0.0)),
+    # large enough for the concurrent sub-tree tasks (>= 1e5 points per task level) and the chunked list build
+    ("cfg1_threaded_build", lambda: I.config1()),
+    ("random_300k_threaded_build", lambda: I.random_cloud(300000, seed=16, leaf_size=400, batch_size=400, degree=5)),
+    ("clustered_250k_second_tree", lambda: I.random_cloud(250000, seed=17, clustered=True, leaf_size=600,
+                                                          batch_size=250, degree=6, theta=0.8)),
 ]
 
 
@@ -108,3 +113,32 @@ def test_bench_flops_table_matches_the_built_sass():
         assert r["R"] == (2 if r["OT"] <= 2 else 1)
         seen.add(key)
     assert seen == set(bench.FLOPS_PER_PAIR)
+
+
+def test_host_plan_fuzz_against_oracle_tree(oracle_mod):
+    # seeded sweep over odd sizes and parameters: tiny N, leaf size 1, exact duplicates, planar and collinear clouds
+    rng = np.random.default_rng(20030183 + 77)
+    for case in range(40):
+        N = int(rng.choice([1, 2, 3, 17, 64, 257, 1000, 2500, 4000]))
+        leaf = int(rng.choice([1, 2, 7, 32, 100, 300]))
+        batch = leaf if rng.random() < 0.6 else int(rng.choice([1, 5, 50, 200]))
+        theta = float(rng.choice([0.0, 0.3, 0.7, 0.95]))
+        degree = int(rng.integers(1, 7))
+        X = rng.random((3, N))
+        shape = rng.integers(0, 4)
+        if shape == 1:
+            X[2] = 0.25                                        # planar: a degenerate box axis (reading R8)
+        elif shape == 2:
+            X[1] = X[0]; X[2] = 0.5                            # collinear
+        elif shape == 3 and N > 3:
+            X[:, N // 2:] = X[:, : N - N // 2]                 # every point duplicated (R3, R5: unsplittable clusters)
+        X = np.ascontiguousarray(X)
+        p = B.bltc_create_host_plan(None, X, None, N, theta, degree, batch, leaf)
+        e = B.bltc_export_plan(p)
+        st = B.bltc_get_stats(p)
+        op = oracle_mod.OraclePlan((X[0], X[1], X[2]), theta, degree, leaf, batch)
+        oe = op.export()
+        for key in e:
+            np.testing.assert_array_equal(e[key], oe[key], err_msg=f"case {case} {key} N={N} leaf={leaf} batch={batch}")
+        assert (st["far_evals"], st["near_evals"]) == (op.far_evals, op.near_evals)
+        B.bltc_destroy(p)
