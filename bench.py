@@ -5,16 +5,22 @@
   python bench.py --impl reference --steps K --warmup W     the CPU oracle, as it stands, on host cores
 
 A "step" is one pass of the whole hot path: one bltc_convolve call for all
-orbitals of the workload = BASELINE.json configs[1] (Be-like atom, adaptive Fejer mesh, 2 orbitals,
-theta 0.7, degree 8, N_L = N_B = 2000).  The plan (a0, host tree build) is built once before the
-timed region and reported separately, as the paper does (stage 1 vs stage 2).
+orbitals of the workload = BASELINE.json configs[3], the largest single-GPU configuration (C6H6-like
+molecule, adaptive Fejer mesh of 3,462,656 points, 21 orbitals, theta 0.7, degree 8, N_L = N_B = 2000;
+PAPER.md:518 is the paper's largest system).  The plan (a0) is built once before the timed region and
+reported separately, as the paper does (stage 1 vs stage 2).  The round-1 workload
+(configs[1]) is timed for a few steps on the same build and reported under "cfg1".
 
-value   = equivalent direct interactions per second = n_orb * N^2 * n_gpus / t_step (inputs in HBM)
+value   = equivalent direct interactions per second = n_orb * N^2 / t_step (inputs in HBM)
 e2e     = the same through the C ABI with HOST (pinned) buffers: H2D of f and D2H of out inside the
-          timed region
-roofline= FP64 ALU bound: executed FP64 flops of the dominant kernel / its CUDA-event time / FP64 peak
-Multi-GPU: the path does not need to shard on one node ("replicas only"): every rank runs
-the same convolution on its own GPU (weak scaling), no data-path collective.
+          timed region (min(K, 5) steps: a step is ~17 s)
+roofline= FP64 ALU bound: executed FP64 flops of the pair kernel that dominates the step / its CUDA-event
+          time / FP64 peak; the other pair kernel is reported beside it
+cpu_baseline / cpu_baseline_fast = the CPU oracle (strict build = the parity oracle; -O3 -march=native
+          -ffast-math build of the same sources) on a bounded sample, all host cores busy
+Multi-GPU (--gpus N > 1): target batches are sharded over the ranks (strong scaling, one convolution),
+the ranks' slices of `out` are all-gathered over NCCL; --shard replicas: every rank
+convolves its own orbitals on the same mesh (weak scaling, no collective).
 """
 from __future__ import annotations
 
@@ -51,6 +57,14 @@ FLOPS_PER_PAIR = {
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.
 FP64_PEAK_TFLOPS_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def measured_hbm_gbs():
+    """MEASURED_PEAKS.json's copy bandwidth (driver-written), else the profiling guide's fallback."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        return 6650.0
 
 
 def orbital_groups(n_orb, max_ot=4):
@@ -129,55 +143,84 @@ def workload(name="cfg1", kernel="yukawa", orbitals=0):
 
 
 def sample_batches(n_batches, count=4):
-    """Evenly spread batch ids; cfg1 (568 batches) keeps the ids the earlier rounds used."""
-    if n_batches == 568:
-        return [0, 137, 301, 567][:count]
+    """Evenly spread batch ids."""
     return sorted(set(int(round(i * (n_batches - 1) / max(count - 1, 1))) for i in range(count)))
 
 
-def cpu_oracle_sample(c, batches, repeat=1, kernel="yukawa"):
-    """Time the CPU oracle's BLTC (as it stands) on a bounded sample of target batches and scale to the
-    whole convolution by evaluation count.  Returns (equiv. interactions/s, seconds, description)."""
+CPU_SAMPLE_BATCHES = 4      # both CPU legs (cpu_baseline inside the CUDA arm, --impl reference) time this sample
+
+
+def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
+    """Time the CPU oracle's BLTC (as it stands) on a bounded sample of the workload -- CPU_SAMPLE_BATCHES evenly
+    spread target batches, the first orbital -- and scale to the whole convolution phase by phase: the proxy-charge
+    phase (Alg. 3 line 2) by particle-cluster pairs, the batch-cluster sums (line 3) by kernel evaluations, both times
+    n_orb.  (A few batches need the proxy charges of a large share of all clusters, so scaling the whole sample by
+    evaluation count alone would charge the CPU for upward passes it does once per convolution.)  The oracle's loops
+    are parallel over clusters and over targets: every core is busy.  fast=True: the same sources built
+    -O3 -march=native -ffast-math (oracle/liboracle_fast.so; timing only, never used for parity).
+    Returns (equiv. interactions/s, seconds of the sample, description, threads)."""
     import oracle
-    op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size, fast=fast)
     e = op.export()
     size = e["cl_end"] - e["cl_begin"]
-    ev = 0
-    if isinstance(batches, int):
-        batches = sample_batches(op.n_batches, batches)
+    batches = sample_batches(op.n_batches, CPU_SAMPLE_BATCHES)
+    ev, need = 0, set()
     for b in batches:
         nt = e["b_end"][b] - e["b_begin"][b]
         ev += nt * (op.P * (e["far_ptr"][b + 1] - e["far_ptr"][b])
                     + size[e["near_idx"][e["near_ptr"][b]:e["near_ptr"][b + 1]]].sum())
-    total = op.far_evals + op.near_evals
+        need.update(e["far_idx"][e["far_ptr"][b]:e["far_ptr"][b + 1]].tolist())
+    up_sample = int(size[sorted(need)].sum()) if need else 0
+    up_total = int(size[np.unique(e["far_idx"])].sum()) if len(e["far_idx"]) else 0
+    ev_total = op.far_evals + op.near_evals
     best = None
     for _ in range(repeat):
         t0 = time.perf_counter()
         if kernel == "coulomb":
-            op.evaluate_coulomb(c.w, c.f, alpha=1.0, batches=list(batches))
+            op.evaluate_coulomb(c.w, c.f[:1], alpha=1.0, batches=batches)
         else:
-            op.evaluate(c.w, c.f, c.k, batches=list(batches))
+            op.evaluate(c.w, c.f[:1], c.k[:1], batches=batches)
         dt = time.perf_counter() - t0
-        best = dt if best is None else min(best, dt)
-    t_full = best * total / ev                       # seconds for all batches, all orbitals
+        if best is None or dt < best[0]:
+            best = (dt, op.phase_seconds[0], op.phase_seconds[1])
+    dt, t_up, t_ev = best
+    t_full = c.n_orb * ((t_up * up_total / up_sample if up_sample else 0.0) + t_ev * ev_total / ev)
     value = c.n_orb * float(c.N) ** 2 / t_full
     ntg = int(sum(e["b_end"][b] - e["b_begin"][b] for b in batches))
-    desc = (f"CPU BLTC oracle (oracle/bltc_cpu.c, strict IEEE, long-double sums) on {len(batches)} of "
-            f"{op.n_batches} target batches ({ntg} targets, {c.n_orb} orbitals, {ev * c.n_orb:.3g} kernel "
-            f"evaluations incl. their proxy charges), {best:.2f} s, scaled by evaluation count to the "
-            f"whole convolution")
-    return value, best, desc, oracle.n_threads()
+    threads = oracle.n_threads()
+    build = ("-O3 -march=native -ffast-math build of the same sources (timing only)" if fast
+             else "strict IEEE build, long-double sums: the parity oracle")
+    desc = (f"CPU BLTC oracle (oracle/bltc_cpu.c, {build}) on {len(batches)} of {op.n_batches} target batches "
+            f"({ntg} targets) x 1 of {c.n_orb} orbitals, {threads} OpenMP threads over clusters / targets: "
+            f"{t_up:.2f} s proxy charges ({up_sample:.3g} of {up_total:.3g} particle-cluster pairs) + {t_ev:.2f} s "
+            f"batch sums ({ev:.3g} of {ev_total:.3g} kernel evaluations); each phase scaled by its count, x n_orb")
+    return value, dt, desc, threads
+
+
+def config_dict(c, args, world):
+    """The `config` object of the JSON line -- the same for the CUDA arm and the reference arm."""
+    coulomb = args.kernel == "coulomb"
+    sharded = args.shard == "batches" and world > 1
+    return {"workload": c.name + (f" (BASELINE.json configs[{args.workload[3:]}])" if not coulomb and not args.orbitals else ""),
+            "kernel": "coulomb 1/r, Gaussian subtraction alpha = 1 (Eq. (23)-(24))" if coulomb
+            else "yukawa e^{-kr}/(4 pi r), subtraction Eq. (20)-(21)", "N": c.N, "n_orb": c.n_orb, "theta": c.theta,
+            "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
+            "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
+            "parallelism": ("1 GPU" if world == 1 else
+                            f"target batches sharded over {world} ranks + all-gather of out (NCCL)" if sharded
+                            else f"{world} replicas (each rank its own orbitals), no collective")}
 
 
 def run_reference(args):
+    """The reference arm of this tier: the CPU oracle, as it stands, on the host cores -- every step times the
+    same bounded sample as the CUDA arm's cpu_baseline leg."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     c = workload(args.workload, args.kernel, args.orbitals)
-    batches = [137] if args.workload == "cfg1" else 1
     vals = []
     for i in range(args.warmup + args.steps):
-        v, dt, desc, cores = cpu_oracle_sample(c, batches, kernel=args.kernel)
+        v, dt, desc, cores = cpu_oracle_sample(c, kernel=args.kernel)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
@@ -185,16 +228,50 @@ def run_reference(args):
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": c.name, "N": c.N, "n_orb": c.n_orb, "theta": c.theta, "degree": c.degree,
-                   "leaf_size": c.leaf_size, "batch_size": c.batch_size,
-                   "note": "each step = the CPU oracle on a bounded sample of the workload"},
+        "scaling": "strong" if args.shard == "batches" and args.gpus > 1 else "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": config_dict(c, args, args.gpus),
+        "note": "each step = the CPU oracle on a bounded sample of the workload (see cpu_baseline.sample)",
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
     return 0
+
+
+def roofline_of(phase_ms, st, groups, degree, coulomb, probe, steps):
+    """FP64-ALU roofline of the two pair kernels from the library's per-phase CUDA events: executed FP64 flops
+    (SASS-counted mix x the plan's exact pair counts, summed over the orbital groups of one step) / kernel time."""
+    pre = "c" if coulomb else ""
+    far_key = pre + ("far9" if degree == 8 else "far")
+    peak = FP64_PEAK_TFLOPS_NOMINAL
+    out = {}
+    for name, key, evals in (("near", pre + "near", st["near_evals"]), ("far", far_key, st["far_evals"])):
+        ms = phase_ms[name] / steps                      # all launches of one step
+        flops = sum(evals * FLOPS_PER_PAIR[(key, g)] for g in groups)
+        tf = flops / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        out[name] = {"bound": "alu", "kernel": name + "_kernel", "achieved": tf, "peak": peak, "unit": "TFLOP/s",
+                     "frac": tf / peak, "frac_of_measured_dfma_probe": tf / probe if probe else None,
+                     "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md 6)",
+                     "peak_measured_dfma_probe": probe, "launches_per_step": len(groups),
+                     "orbital_tiles": groups, "avg_launch_ms": ms / len(groups),
+                     "flops_per_launch": flops / len(groups), "ms_per_step": ms}
+    return out
+
+
+def committed_traffic(workload_name, kernel):
+    """DRAM bytes of one launch of `kernel` on this workload from the committed ncu capture (profiles/r02_traffic.csv:
+    workload,kernel,dram_bytes_per_launch -- profiles/r02_traffic.md names the command); None if not captured."""
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    try:
+        for line in open(tpath):
+            p = [x.strip() for x in line.split(",")]
+            if len(p) >= 3 and p[0] == workload_name and p[1] == kernel:
+                return float(p[2])
+    except Exception:
+        pass
+    return None
 
 
 def run_cuda(args):
@@ -209,100 +286,128 @@ def run_cuda(args):
         raise SystemExit("bench.py: no CUDA device -- the product has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator log (NVLS / ring) stays on
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
 
-    c = workload(args.workload, args.kernel, args.orbitals)
     coulomb = args.kernel == "coulomb"
-    N, O = c.N, c.n_orb
-
-    def convolve(f_, out_):
-        if coulomb:
-            B.bltc_convolve_coulomb(plan, f_, O, out_, True, 1.0)
-        else:
-            B.bltc_convolve(plan, c.k, f_, O, out_, True)
-        if exchange is not None and out_.is_cuda:
-            exchange.all_gather_out(out_)
-
-    X = torch.from_numpy(c.coords()).cuda()
-    w = torch.from_numpy(c.w).cuda()
-    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
-    out = torch.zeros((O, N), dtype=torch.float64, device="cuda")      # a sharded plan writes its slice only
-    t0 = time.perf_counter()
     sharded = args.shard == "batches" and world > 1
-    exchange = None
-    if sharded:      # strong scaling: rank r computes its slice of the target batches; the only exchange is the
-        # all-gather of `out` that the next Green-Iteration step needs on every rank
-        from paper_2003_01833_b200.multi_gpu import ShardExchange
-        plan = B.bltc_create_sharded(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
-        exchange = ShardExchange(B.bltc_get_shard_targets(plan), N, "cuda")
-    else:
-        plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
-    create_ms = (time.perf_counter() - t0) * 1e3
-    st = B.bltc_get_stats(plan)
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")   # > 126 MB L2
+    warmup = max(args.warmup, 3)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    groups = orbital_groups(O)
-    launches_per_step = int(st["launches_per_group"]) * len(groups)
+    def max_over_ranks(v):
+        if world > 1:
+            t = torch.tensor([v], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return v
 
-    # ---- device-resident timing -------------------------------------------------------------
-    B.bltc_set_profiling(plan, True)
-    for _ in range(max(args.warmup, 3)):
-        convolve(f, out)
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    phase_sum = {p: 0.0 for p in B.PHASES}
-    barrier()
-    for i in range(args.steps):
-        flush.fill_(0.0)                                        # L2 flush between timed iterations
-        ev[i][0].record(stream)
-        convolve(f, out)
-        ev[i][1].record(stream)
-        ph = B.bltc_get_phase_ms(plan)                          # syncs on the step's last event
-        for p in B.PHASES:
-            phase_sum[p] += ph[p]
-    barrier()
-    clocks = sampler.stop()
-    t_ms = sum(a.elapsed_time(b) for a, b in ev)
-    if world > 1:
-        t = torch.tensor([t_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_ms = float(t.item())
-    ms_per_step = t_ms / args.steps
+    def time_workload(c, steps, warm, shard, e2e_steps, sample_clocks):
+        """Plan + `steps` timed convolutions (device-resident) + `e2e_steps` through host buffers."""
+        N, O = c.N, c.n_orb
+        X = torch.from_numpy(c.coords()).cuda()
+        w = torch.from_numpy(c.w).cuda()
+        f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+        out = torch.zeros((O, N), dtype=torch.float64, device="cuda")      # a sharded plan writes its slice only
+        exchange = None
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        if shard:    # strong scaling: rank r computes its slice of the target batches; the only exchange is the
+            # all-gather of `out` that the next Green-Iteration step needs on every rank (DESIGN.md 9.2)
+            from paper_2003_01833_b200.multi_gpu import ShardExchange
+            plan = B.bltc_create_sharded(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
+            exchange = ShardExchange(B.bltc_get_shard_targets(plan), N, "cuda")
+        else:
+            plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
+        create_ms = (time.perf_counter() - t0) * 1e3
+        st = B.bltc_get_stats(plan)
+
+        def convolve(f_, out_):
+            if coulomb:
+                B.bltc_convolve_coulomb(plan, f_, O, out_, True, 1.0)
+            else:
+                B.bltc_convolve(plan, c.k, f_, O, out_, True)
+            if exchange is not None:
+                exchange.all_gather_out(out_)
+
+        # ---- device-resident timing ---------------------------------------------------------
+        B.bltc_set_profiling(plan, True)
+        for _ in range(warm):
+            convolve(f, out)
+        barrier()
+        sampler = ClockSampler(local) if sample_clocks else None
+        if sampler:
+            sampler.start()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        phase_sum = {p: 0.0 for p in B.PHASES}
+        barrier()
+        for i in range(steps):
+            flush.fill_(0.0)                                        # L2 flush between timed iterations
+            ev[i][0].record(stream)
+            convolve(f, out)
+            ev[i][1].record(stream)
+            ph = B.bltc_get_phase_ms(plan)                          # syncs on the step's last event
+            for p in B.PHASES:
+                phase_sum[p] += ph[p]
+        barrier()
+        clocks = sampler.stop() if sampler else None
+        ms_per_step = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev)) / steps
+
+        # ---- end to end through the C ABI with host (pinned) buffers ----------------------------
+        B.bltc_set_profiling(plan, False)
+        e2e = None
+        if e2e_steps > 0:
+            f_host = torch.from_numpy(np.ascontiguousarray(c.f)).pin_memory()
+            out_host = torch.zeros((O, N), dtype=torch.float64).pin_memory()
+            out_dev = torch.zeros((O, N), dtype=torch.float64, device="cuda") if exchange is not None else None
+
+            def convolve_host():            # H2D(f) + a1..a5 + D2H(out) + stream sync, all inside the C call
+                if coulomb:
+                    B.bltc_convolve_coulomb(plan, f_host, O, out_host, True, 1.0)
+                else:
+                    B.bltc_convolve(plan, c.k, f_host, O, out_host, True)
+                if exchange is not None:    # sharded: the ranks' slices are exchanged on the device
+                    out_dev.copy_(out_host, non_blocking=True)
+                    exchange.all_gather_out(out_dev)
+
+            convolve_host()
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e2e_ms = 0.0
+            for i in range(e2e_steps):
+                flush.fill_(0.0)
+                e0.record(stream)
+                convolve_host()
+                e1.record(stream)
+                e1.synchronize()
+                e2e_ms += e0.elapsed_time(e1)
+            barrier()
+            e2e_ms = max_over_ranks(e2e_ms) / e2e_steps
+            res = out_dev if exchange is not None else torch.from_numpy(out_host.numpy())
+            same = bool(torch.equal(res.cpu(), out.cpu()))
+            e2e = {"ms_per_step": e2e_ms, "steps": e2e_steps, "bitwise_equal_to_device_path": same}
+        return dict(plan=plan, st=st, X=X, w=w, f=f, out=out, ms_per_step=ms_per_step, phase_sum=phase_sum,
+                    create_ms=create_ms, clocks=clocks, e2e=e2e)
+
+    # ---- the headline workload ----------------------------------------------------------------
+    c = workload(args.workload, args.kernel, args.orbitals)
+    N, O = c.N, c.n_orb
+    e2e_steps = min(args.steps, 5)
+    R = time_workload(c, args.steps, warmup, sharded, e2e_steps, True)
+    plan, st, X, w, f, out = R["plan"], R["st"], R["X"], R["w"], R["f"], R["out"]
+    ms_per_step = R["ms_per_step"]
     jobs = 1 if sharded else world          # replicas: every rank convolves its own orbitals on the same mesh
     value = jobs * O * float(N) ** 2 / (ms_per_step * 1e-3)
-
-    # ---- end to end through the C ABI with host buffers ------------------------------------
-    B.bltc_set_profiling(plan, False)
-    f_host = torch.from_numpy(np.ascontiguousarray(c.f)).pin_memory()
-    out_host = torch.zeros((O, N), dtype=torch.float64).pin_memory()
-    for _ in range(2):
-        convolve(f_host, out_host)
-    barrier()
+    e2e_value = jobs * O * float(N) ** 2 / (R["e2e"]["ms_per_step"] * 1e-3)
+    groups = orbital_groups(O)
+    launches_per_step = int(st["launches_per_group"]) * len(groups)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e2e_ms = 0.0
-    for i in range(args.steps):
-        flush.fill_(0.0)
-        e0.record(stream)
-        convolve(f_host, out_host)                              # H2D(f) + a1..a5 + D2H(out) + stream sync
-        e1.record(stream)
-        e1.synchronize()
-        e2e_ms += e0.elapsed_time(e1)
-    barrier()
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = jobs * O * float(N) ** 2 / (e2e_ms / args.steps * 1e-3)
-    same = bool(np.array_equal(out_host.numpy(), out.cpu().numpy()))
 
     # ---- a6: brute-force direct sum (SURVEY.md 8(a) a6) on a bounded target sample of this workload --------
     direct = None
@@ -315,7 +420,7 @@ def run_cuda(args):
         dout = torch.empty((O, M), dtype=torch.float64, device="cuda")
         B.bltc_direct_set_profiling(True)
         d_ms, d_total = [], []
-        for i in range(2 + 5):
+        for i in range(1 + 3):
             flush.fill_(0.0)
             e0.record(stream)
             if coulomb:
@@ -324,16 +429,15 @@ def run_cuda(args):
                 B.direct_convolve(Tg, fT, M, X, w, f, N, c.k, O, dout, True)
             e1.record(stream)
             e1.synchronize()
-            if i >= 2:
+            if i >= 1:
                 d_ms.append(B.bltc_direct_get_kernel_ms()); d_total.append(e0.elapsed_time(e1))
         B.bltc_direct_set_profiling(False)
         dk = float(np.median(d_ms))
-        d_flops = sum(float(M) * N * FLOPS_PER_PAIR[(("c" if coulomb else "") + "near", g)] for g in orbital_groups(O))
+        d_flops = sum(float(M) * N * FLOPS_PER_PAIR[(("c" if coulomb else "") + "near", g)] for g in groups)
         direct = {"targets": M, "sources": N, "n_orb": O, "pair_kernel_ms": dk, "call_ms": float(np.median(d_total)),
                   "pairs_per_s": O * float(M) * N / (dk * 1e-3), "tflops": d_flops / (dk * 1e-3) / 1e12,
                   "frac": d_flops / (dk * 1e-3) / 1e12 / FP64_PEAK_TFLOPS_NOMINAL,
-                  "note": "direct_convolve on a seeded target sample (same pair kernel as the near field, "
-                          "r == 0 test and underflow guard compiled in)"}
+                  "note": "direct_convolve on a seeded target sample (the near field's pair kernel over all sources)"}
 
     # ---- NEXT-2: Green-Iteration epilogue (Alg. 2 lines 4-7) on this mesh, HBM-bound ------------------
     gi = None
@@ -356,70 +460,62 @@ def run_cuda(args):
         gi_bytes = (11 + 2 * n_prev) * 8 * N          # K1 reads 4+n, K2 reads 2+n writes 1, K3 reads 3 writes 1
         gi_t = float(np.median(gi_ms))
         gi = {"ms": gi_t, "n_prev": n_prev, "launches": 4, "algorithmic_bytes": gi_bytes,
-              "GBps": gi_bytes / (gi_t * 1e-3) / 1e9, "note": "L2 flushed before each call; 4 small kernels: launch-latency bound at this N"}
+              "GBps": gi_bytes / (gi_t * 1e-3) / 1e9, "hbm_peak_GBps_measured": measured_hbm_gbs(),
+              "note": "L2 flushed before each call; 4 dependent streaming kernels"}
+        del phi, psi_old
+    probe = B.bltc_probe_fp64(64) if rank == 0 else None
+    stq = dict(st, near_evals=st["shard_near_evals"], far_evals=st["shard_far_evals"]) if sharded else st
+    roof = roofline_of(R["phase_sum"], stq, groups, c.degree, coulomb, probe, args.steps) if rank == 0 else None
+    phase_ms = {p: v / args.steps for p, v in R["phase_sum"].items()}
+    create_ms, clocks, e2e_info = R["create_ms"], R["clocks"], R["e2e"]
+    B.bltc_destroy(plan)
+    del X, w, f, out, R
+
+    # ---- context: the round-1 bench workload (configs[1]) on the same build, a few steps -----------------
+    cfg1 = None
+    if rank == 0 and world == 1 and args.workload == "cfg3" and not coulomb and not args.orbitals:
+        c1 = workload("cfg1", args.kernel, 0)
+        R1 = time_workload(c1, 5, 3, False, 0, False)
+        r1 = roofline_of(R1["phase_sum"], R1["st"], orbital_groups(c1.n_orb), c1.degree, False, probe, 5)
+        cfg1 = {"workload": c1.name, "N": c1.N, "n_orb": c1.n_orb, "ms_per_step": R1["ms_per_step"],
+                "value": c1.n_orb * float(c1.N) ** 2 / (R1["ms_per_step"] * 1e-3), "steps": 5,
+                "near_frac": r1["near"]["frac"], "far_frac": r1["far"]["frac"],
+                "plan_create_ms": R1["create_ms"]}
+        B.bltc_destroy(R1["plan"])
+        del R1
 
     if rank == 0:
-        near_ms = phase_sum["near"] / args.steps / len(groups)      # average launch duration
-        far_ms = phase_sum["far"] / args.steps / len(groups)
-        pre = "c" if coulomb else ""
-        if sharded:                          # rank 0's kernels work on rank 0's slice
-            st = dict(st, near_evals=st["shard_near_evals"], far_evals=st["shard_far_evals"])
-        near_flops = sum(st["near_evals"] * FLOPS_PER_PAIR[(pre + "near", g)] for g in groups) / len(groups)
-        far_key = pre + ("far9" if c.degree == 8 else "far")
-        far_flops = sum(st["far_evals"] * FLOPS_PER_PAIR[(far_key, g)] for g in groups) / len(groups)
-        peak = FP64_PEAK_TFLOPS_NOMINAL
-        near_tf = near_flops / (near_ms * 1e-3) / 1e12
-        far_tf = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
-        probe = B.bltc_probe_fp64(64)
-        # DRAM bytes of one near-kernel launch of THIS workload from the committed ncu capture
-        # (profiles/r01g_summary.md names the command); null for other workloads / kernels
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r01g_near_cfg1_dram.csv")
-        if args.workload == "cfg1" and not coulomb and os.path.exists(tpath):
-            try:
-                import csv
-                rows = [r for r in csv.reader(open(tpath)) if len(r) > 5 and r[-3].startswith("dram__bytes")]
-                traffic = float(sum(float(r[-1].replace(",", "")) for r in rows)) if rows else None
-            except Exception:
-                traffic = None
-        cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, 4, kernel=args.kernel)
+        dom = "near" if roof["near"]["ms_per_step"] >= roof["far"]["ms_per_step"] else "far"
+        other = "far" if dom == "near" else "near"
+        roof[dom]["traffic"] = committed_traffic(args.workload if not args.orbitals else "", dom + "_kernel")
+        cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, kernel=args.kernel)
+        fast_v, fast_dt, fast_desc, fast_cores = cpu_oracle_sample(c, kernel=args.kernel, fast=True)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": c.name + (" (BASELINE.json configs[1])" if args.workload == "cfg1" and not coulomb else ""),
-                       "kernel": "coulomb 1/r, Gaussian subtraction alpha = 1 (Eq. (23)-(24))" if coulomb
-                       else "yukawa e^{-kr}/(4 pi r), subtraction Eq. (20)-(21)", "N": N, "n_orb": O, "theta": c.theta,
-                       "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
-                       "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
-                       "parallelism": ("1 GPU" if world == 1 else
-                                       f"target batches sharded over {world} ranks + all-gather of out (NCCL)" if sharded
-                                       else f"{world} replicas (each rank its own orbitals), no collective")},
+            "config": config_dict(c, args, world),
             "time_per_convolution_ms": ms_per_step / O,
-            "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * world / (ms_per_step * 1e-3),
-            "phase_ms": {p: phase_sum[p] / args.steps for p in B.PHASES},
+            "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * jobs / (ms_per_step * 1e-3),
+            "phase_ms": phase_ms,
             "plan": {"create_ms": create_ms, "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
                      "clusters": st["n_clusters"], "batches": st["n_batches"],
                      "far_evals": st["far_evals"], "near_evals": st["near_evals"]},
-            "roofline": {"bound": "alu", "kernel": "near_kernel", "achieved": near_tf, "peak": peak,
-                         "unit": "TFLOP/s", "frac": near_tf / peak, "traffic": traffic,
-                         "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md)",
-                         "peak_measured_dfma_probe": probe, "avg_launch_ms": near_ms,
-                         "flops_per_launch": near_flops},
-            "roofline_far": {"bound": "alu", "kernel": "far_kernel", "achieved": far_tf, "peak": peak,
-                             "unit": "TFLOP/s", "frac": far_tf / peak, "avg_launch_ms": far_ms,
-                             "flops_per_launch": far_flops},
+            "roofline": roof[dom], "roofline_" + other: roof[other],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": O * N * 8,
-                    "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_ms / args.steps,
-                    "bitwise_equal_to_device_path": same},
+                    "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_info["ms_per_step"],
+                    "steps": e2e_info["steps"],
+                    "bitwise_equal_to_device_path": e2e_info["bitwise_equal_to_device_path"]},
             "direct": direct,
             "gi_update": gi,
+            "cfg1": cfg1,
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks,
             "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},
+            "cpu_baseline_fast": {"value": fast_v, "unit": UNIT, "cores": fast_cores, "kind": "oracle, fast-math build",
+                                  "sample": fast_desc},
         }
         print(json.dumps(line))
-    B.bltc_destroy(plan)
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -431,11 +527,12 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "batches"],
-                    help="N > 1: replicas = each rank convolves its own orbitals (weak scaling, default); "
-                         "batches = one convolution, target batches sharded over the ranks (strong scaling)")
-    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"],
-                    help="cfg1 = BASELINE.json configs[1] (the bench line); others: profiling / context")
+    ap.add_argument("--shard", default="batches", choices=["replicas", "batches"],
+                    help="N > 1: batches = one convolution, target batches sharded over the ranks + all-gather of out "
+                         "(strong scaling, default); replicas = each rank convolves its own orbitals (weak scaling)")
+    ap.add_argument("--workload", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"],
+                    help="cfg3 = BASELINE.json configs[3], the largest single-GPU config (the bench line); "
+                         "others: profiling / context")
     ap.add_argument("--orbitals", type=int, default=0,
                     help="profiling aid: cycle the workload's fields to this many orbitals (0 = as configured)")
     ap.add_argument("--kernel", default="yukawa", choices=["yukawa", "coulomb"],

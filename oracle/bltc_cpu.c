@@ -38,6 +38,7 @@
  * -ffp-contract=off); every sum over particles or interpolation points in long double.
  */
 #include <math.h>
+#include <omp.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -382,6 +383,14 @@ int oracle_plan_proxy(const oracle_plan* p, int c, const double* q_caller, doubl
     return 0;
 }
 
+/* threads the parallel loops below use (reported beside the timed baseline) */
+int oracle_max_threads(void) { return omp_get_max_threads(); }
+
+/* wall-clock seconds of the last evaluation's two phases: [0] proxy charges (Alg. 3 line 2), [1] batch-cluster sums
+ * (line 3).  Timing only -- bench.py scales a sampled run to the whole convolution phase by phase. */
+static double g_phase_s[2];
+void oracle_last_phase_seconds(double out[2]) { out[0] = g_phase_s[0]; out[1] = g_phase_s[1]; }
+
 /* ------------------------------------------------------------------ evaluation */
 /* One orbital.  w, f_src: [N] caller order.  f_tgt: [M] caller order (NULL unless subtract;
  * when targets are the sources pass f_tgt = f_src).  sel: batch ids to evaluate (NULL = all);
@@ -408,6 +417,7 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
     double* fw = (double*)malloc((size_t)p->N * sizeof(double));
     for (int64_t j = 0; j < p->N; ++j) fw[j] = f_src[j] * w[j];
     int c;
+    double t_phase0 = omp_get_wtime();
 #pragma omp parallel for schedule(dynamic, 1)
     for (c = 0; c < ncl; ++c) {
         if (!need[c]) continue;
@@ -416,11 +426,22 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
         if (subtract) { what[c] = (double*)malloc((size_t)P * sizeof(double)); proxy_charges(p, c, w, what[c]); }
     }
     /* line 3: for each target batch, the recorded batch-cluster interactions */
-    int64_t s;
-#pragma omp parallel for schedule(dynamic, 1)
-    for (s = 0; s < nb; ++s) {
+    /* Targets are independent (each one's sums are accumulated by one thread, in the order written below), so the
+     * threads share the flat list of the selected batches' targets -- a sample of a few batches keeps every core busy. */
+    int64_t ntg = 0, u;
+    for (int64_t s = 0; s < nb; ++s) { int64_t b = sel ? sel[s] : s; ntg += p->bend[b] - p->bbegin[b]; }
+    int64_t* tg_it = (int64_t*)malloc((size_t)(ntg ? ntg : 1) * sizeof(int64_t));
+    int64_t* tg_b = (int64_t*)malloc((size_t)(ntg ? ntg : 1) * sizeof(int64_t));
+    ntg = 0;
+    for (int64_t s = 0; s < nb; ++s) {
         int64_t b = sel ? sel[s] : s;
-        for (int64_t it = p->bbegin[b]; it < p->bend[b]; ++it) {
+        for (int64_t it = p->bbegin[b]; it < p->bend[b]; ++it) { tg_it[ntg] = it; tg_b[ntg] = b; ++ntg; }
+    }
+    double t_phase1 = omp_get_wtime();
+#pragma omp parallel for schedule(dynamic, 16)
+    for (u = 0; u < ntg; ++u) {
+        {
+            int64_t b = tg_b[u], it = tg_it[u];
             int64_t i = p->tperm[it];
             double xi = p->tx[i], yi = p->ty[i], zi = p->tz[i];
             double fi = subtract ? f_tgt[i] : 0.0;
@@ -459,8 +480,9 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
             } else out[i] = (double)S;
         }
     }
+    g_phase_s[0] = t_phase1 - t_phase0; g_phase_s[1] = omp_get_wtime() - t_phase1;
     for (c = 0; c < ncl; ++c) { free(fhat[c]); free(what[c]); }
-    free(fhat); free(what); free(fw); free(need);
+    free(fhat); free(what); free(fw); free(need); free(tg_it); free(tg_b);
     return 0;
 }
 
@@ -497,6 +519,7 @@ int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double
     double* fw = (double*)malloc((size_t)p->N * sizeof(double));
     for (int64_t j = 0; j < p->N; ++j) fw[j] = f_src[j] * w[j];
     int c;
+    double t_phase0 = omp_get_wtime();
 #pragma omp parallel for schedule(dynamic, 1)
     for (c = 0; c < ncl; ++c) {
         if (!need[c]) continue;
@@ -504,11 +527,22 @@ int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double
         proxy_charges(p, c, fw, fhat[c]);
         if (subtract) { what[c] = (double*)malloc((size_t)P * sizeof(double)); proxy_charges(p, c, w, what[c]); }
     }
-    int64_t s;
-#pragma omp parallel for schedule(dynamic, 1)
-    for (s = 0; s < nb; ++s) {
+    /* Targets are independent (each one's sums are accumulated by one thread, in the order written below), so the
+     * threads share the flat list of the selected batches' targets -- a sample of a few batches keeps every core busy. */
+    int64_t ntg = 0, u;
+    for (int64_t s = 0; s < nb; ++s) { int64_t b = sel ? sel[s] : s; ntg += p->bend[b] - p->bbegin[b]; }
+    int64_t* tg_it = (int64_t*)malloc((size_t)(ntg ? ntg : 1) * sizeof(int64_t));
+    int64_t* tg_b = (int64_t*)malloc((size_t)(ntg ? ntg : 1) * sizeof(int64_t));
+    ntg = 0;
+    for (int64_t s = 0; s < nb; ++s) {
         int64_t b = sel ? sel[s] : s;
-        for (int64_t it = p->bbegin[b]; it < p->bend[b]; ++it) {
+        for (int64_t it = p->bbegin[b]; it < p->bend[b]; ++it) { tg_it[ntg] = it; tg_b[ntg] = b; ++ntg; }
+    }
+    double t_phase1 = omp_get_wtime();
+#pragma omp parallel for schedule(dynamic, 16)
+    for (u = 0; u < ntg; ++u) {
+        {
+            int64_t b = tg_b[u], it = tg_it[u];
             int64_t i = p->tperm[it];
             double xi = p->tx[i], yi = p->ty[i], zi = p->tz[i];
             double fi = subtract ? f_tgt[i] : 0.0;
@@ -546,7 +580,8 @@ int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double
             out[i] = (double)S;
         }
     }
+    g_phase_s[0] = t_phase1 - t_phase0; g_phase_s[1] = omp_get_wtime() - t_phase1;
     for (c = 0; c < ncl; ++c) { free(fhat[c]); free(what[c]); }
-    free(fhat); free(what); free(fw); free(need);
+    free(fhat); free(what); free(fw); free(need); free(tg_it); free(tg_b);
     return 0;
 }

@@ -17,28 +17,39 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 # strict IEEE: no fast-math, no FMA contraction, baseline x86-64 (no -march=native)
 _CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
            "-fno-fast-math", "-Wall"]
+# The same sources as a compiler would build them for speed (the "fair" CPU number).  Used ONLY by
+# bench.py's cpu_baseline_fast key -- never for parity: fast-math changes the arithmetic.
+_LIB_FAST = os.path.join(_HERE, "liboracle_fast.so")
+_CFLAGS_FAST = ["-O3", "-march=native", "-ffast-math", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-Wall"]
 
 _lib = None
+_lib_fast = None
 _dp = C.POINTER(C.c_double)
 _ip64 = C.POINTER(C.c_int64)
 _ip32 = C.POINTER(C.c_int32)
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc if the .so is missing or older than its sources."""
-    stale = force or not os.path.exists(_LIB) or any(
-        os.path.getmtime(s) > os.path.getmtime(_LIB) for s in _SRC)
+def build(force: bool = False, fast: bool = False) -> str:
+    """Compile the oracle with gcc if the .so is missing or older than its sources.  fast=True: the
+    -O3 -march=native -ffast-math build (timing only; -march=native: build it on the machine that runs it)."""
+    target, flags = (_LIB_FAST, _CFLAGS_FAST) if fast else (_LIB, _CFLAGS)
+    stale = force or not os.path.exists(target) or any(
+        os.path.getmtime(s) > os.path.getmtime(target) for s in _SRC)
     if stale:
-        cmd = ["gcc", *_CFLAGS, "-o", _LIB, *_SRC, "-lm"]
+        cmd = ["gcc", *flags, "-o", target, *_SRC, "-lm"]
         subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
-    return _LIB
+    return target
 
 
-def _load():
-    global _lib
-    if _lib is not None:
+def _load(fast: bool = False):
+    global _lib, _lib_fast
+    if fast and _lib_fast is not None:
+        return _lib_fast
+    if not fast and _lib is not None:
         return _lib
-    lib = C.CDLL(build())
+    lib = C.CDLL(build(force=fast, fast=fast))      # the fast build is always rebuilt for this host's CPU
+    lib.oracle_max_threads.restype = C.c_int
+    lib.oracle_last_phase_seconds.argtypes = [_dp]
     lib.oracle_kernel.restype = C.c_double
     lib.oracle_kernel.argtypes = [C.c_int, C.c_double] + [C.c_double] * 6 + [C.POINTER(C.c_int)]
     lib.oracle_direct.restype = C.c_int
@@ -63,14 +74,16 @@ def _load():
     lib.oracle_bltc_eval_coulomb.restype = C.c_int
     lib.oracle_bltc_eval_coulomb.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_double, C.c_int,
                                              C.c_int64, _ip64, _dp, _dp]
-    _lib = lib
+    if fast:
+        _lib_fast = lib
+    else:
+        _lib = lib
     return lib
 
 
 def n_threads() -> int:
-    """Threads the OpenMP loops will use (OMP_NUM_THREADS or all cores)."""
-    v = os.environ.get("OMP_NUM_THREADS")
-    return int(v) if v else (os.cpu_count() or 1)
+    """Threads the oracle's OpenMP loops use: omp_get_max_threads() of the loaded library."""
+    return int(_load().oracle_max_threads())
 
 
 def _d(a):
@@ -153,8 +166,8 @@ class OraclePlan:
     """Tree + batches + interaction lists of oracle/bltc_cpu.c (Algorithm 3 line 1 and the
     decisions of line 3), and the evaluation (lines 2-3)."""
 
-    def __init__(self, sources, theta, degree, leaf_size, batch_size, targets=None):
-        lib = _load()
+    def __init__(self, sources, theta, degree, leaf_size, batch_size, targets=None, fast=False):
+        lib = _load(fast)
         self._lib = lib
         self._s = [_d(a) for a in sources]
         self.N = self._s[0][0].shape[0]
@@ -214,15 +227,20 @@ class OraclePlan:
             raise ValueError("bad cluster index")
         return qhat, nodes
 
-    def evaluate(self, w, f_src, k, *, f_tgt=None, subtract=True, finalize=True, kind=0,
-                 batches=None, return_parts=False):
-        """f_src [N] or [n_orb][N]; returns out [M] or [n_orb][M] in caller order (NaN for
-        targets of batches that were not selected)."""
+    def last_phase_seconds(self):
+        """(proxy-charge seconds, batch-sum seconds) of the most recent library call (one field)."""
+        t = np.zeros(2)
+        self._lib.oracle_last_phase_seconds(t.ctypes.data_as(_dp))
+        return float(t[0]), float(t[1])
+
+    def _evaluate(self, call, w, f_src, f_tgt, subtract, batches, return_parts):
+        """Shared marshalling of evaluate / evaluate_coulomb: one library call per field, call(o, pw, pfo, pft,
+        nsel, psel, pout, pparts) -> rc."""
         w_, pw = _d(w)
         f_src = np.asarray(f_src, dtype=np.float64)
         single = f_src.ndim == 1
         F = np.atleast_2d(f_src)
-        K = np.broadcast_to(np.atleast_1d(np.asarray(k, dtype=np.float64)), (F.shape[0],))
+        FT = None
         if subtract:
             if f_tgt is None:
                 if self._t is not None:
@@ -244,56 +262,33 @@ class OraclePlan:
                 fto, pft = _d(FT[o])
             oo = np.full(self.M, np.nan)
             pp = np.full((2, self.M), np.nan) if return_parts else None
-            rc = self._lib.oracle_bltc_eval(self._h, kind, pw, pfo, pft, float(K[o]), int(subtract),
-                                            int(finalize), nsel, psel, oo.ctypes.data_as(_dp),
-                                            pp.ctypes.data_as(_dp) if return_parts else None)
+            rc = call(o, pw, pfo, pft, nsel, psel, oo.ctypes.data_as(_dp),
+                      pp.ctypes.data_as(_dp) if return_parts else None)
             if rc != 0:
-                raise ValueError("oracle_bltc_eval: bad arguments")
+                raise ValueError("oracle BLTC evaluation: bad arguments")
             out[o] = oo
             if return_parts:
                 parts[o] = pp
+            ph = self.last_phase_seconds()
+            self.phase_seconds = [self.phase_seconds[0] + ph[0], self.phase_seconds[1] + ph[1]] if o else list(ph)
         res = out[0] if single else out
         if return_parts:
             return res, (parts[0] if single else parts)
         return res
 
+    def evaluate(self, w, f_src, k, *, f_tgt=None, subtract=True, finalize=True, kind=0,
+                 batches=None, return_parts=False):
+        """f_src [N] or [n_orb][N]; returns out [M] or [n_orb][M] in caller order (NaN for
+        targets of batches that were not selected)."""
+        n_f = np.atleast_2d(np.asarray(f_src)).shape[0]
+        K = np.broadcast_to(np.atleast_1d(np.asarray(k, dtype=np.float64)), (n_f,))
+        call = lambda o, pw, pfo, pft, nsel, psel, pout, pparts: self._lib.oracle_bltc_eval(
+            self._h, kind, pw, pfo, pft, float(K[o]), int(subtract), int(finalize), nsel, psel, pout, pparts)
+        return self._evaluate(call, w, f_src, f_tgt, subtract, batches, return_parts)
+
     def evaluate_coulomb(self, w, f_src, *, f_tgt=None, subtract=True, alpha=1.0, batches=None,
                          return_parts=False):
         """Hartree potential through the treecode (oracle_bltc_eval_coulomb, reading R21)."""
-        w_, pw = _d(w)
-        f_src = np.asarray(f_src, dtype=np.float64)
-        single = f_src.ndim == 1
-        F = np.atleast_2d(f_src)
-        if subtract:
-            if f_tgt is None:
-                if self._t is not None:
-                    raise ValueError("subtract with separate targets needs f_tgt")
-                FT = F
-            else:
-                FT = np.atleast_2d(np.asarray(f_tgt, dtype=np.float64))
-        if batches is not None:
-            sel = np.ascontiguousarray(batches, dtype=np.int64)
-            nsel, psel = sel.shape[0], sel.ctypes.data_as(_ip64)
-        else:
-            nsel, psel = 0, None
-        out = np.full((F.shape[0], self.M), np.nan)
-        parts = np.full((F.shape[0], 2, self.M), np.nan) if return_parts else None
-        for o in range(F.shape[0]):
-            fo, pfo = _d(F[o])
-            pft = None
-            if subtract:
-                fto, pft = _d(FT[o])
-            oo = np.full(self.M, np.nan)
-            pp = np.full((2, self.M), np.nan) if return_parts else None
-            rc = self._lib.oracle_bltc_eval_coulomb(self._h, pw, pfo, pft, float(alpha), int(subtract),
-                                                    nsel, psel, oo.ctypes.data_as(_dp),
-                                                    pp.ctypes.data_as(_dp) if return_parts else None)
-            if rc != 0:
-                raise ValueError("oracle_bltc_eval_coulomb: bad arguments")
-            out[o] = oo
-            if return_parts:
-                parts[o] = pp
-        res = out[0] if single else out
-        if return_parts:
-            return res, (parts[0] if single else parts)
-        return res
+        call = lambda o, pw, pfo, pft, nsel, psel, pout, pparts: self._lib.oracle_bltc_eval_coulomb(
+            self._h, pw, pfo, pft, float(alpha), int(subtract), nsel, psel, pout, pparts)
+        return self._evaluate(call, w, f_src, f_tgt, subtract, batches, return_parts)

@@ -127,7 +127,7 @@ struct bltc_plan_s {
     DevBuf<int64_t> b_partial_base;
     DevBuf<double> slot_nodes, what;
     DevBuf<Range> near_ranges;
-    DevBuf<WorkItem> far_items[2], near_items[2];
+    DevBuf<WorkItem> far_items, near_items;
     DevBuf<UpItem> up_items;
     DevBuf<UpReduce> up_reduce;
     DevBuf<double> up_chunks;                  // chunk-partial proxy charges (sized for kMaxOT)
@@ -292,10 +292,8 @@ int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sou
         BLTC_TRY_OR_FREE(pl->slot_nodes.upload(hp.slot_nodes));
         BLTC_TRY_OR_FREE(pl->far_slots.upload(hp.far_slots));
         BLTC_TRY_OR_FREE(pl->near_ranges.upload(hp.near_ranges));
-        for (int rv = 0; rv < 2; ++rv) {
-            BLTC_TRY_OR_FREE(pl->far_items[rv].upload(hp.far_items[rv]));
-            BLTC_TRY_OR_FREE(pl->near_items[rv].upload(hp.near_items[rv]));
-        }
+        BLTC_TRY_OR_FREE(pl->far_items.upload(hp.far_items));
+        BLTC_TRY_OR_FREE(pl->near_items.upload(hp.near_items));
         // f-independent proxy weights what_k (Eq. (35) right with q_j = w_j)
         BLTC_TRY_OR_FREE(pl->what.ensure(ns * (size_t)hp.P));
         BLTC_TRY_OR_FREE(pl->up_items.upload(hp.up_items));
@@ -333,14 +331,14 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->near_evals = hp.near_evals;
     s->n_proxy_clusters = (int64_t)hp.cluster_of_slot.size();
     s->upward_pairs = hp.upward_pairs;
-    s->n_far_items = (int64_t)hp.far_items[1].size();
-    s->n_near_items = (int64_t)hp.near_items[1].size();
+    s->n_far_items = (int64_t)hp.far_items.size();
+    s->n_near_items = (int64_t)hp.near_items.size();
     s->partial_len = hp.partial_len;
     s->n_upward_items = (int64_t)hp.up_items.size();
     s->n_upward_reduce = (int64_t)hp.up_reduce.size();
     s->launches_per_group = 1 /* gather */ + (hp.shared_order ? 0 : 1) + (hp.up_items.empty() ? 0 : 1) +
-                            (hp.up_reduce.empty() ? 0 : 1) + (hp.far_items[1].empty() ? 0 : 1) +
-                            (hp.near_items[1].empty() ? 0 : 1) + 1 /* epilogue */;
+                            (hp.up_reduce.empty() ? 0 : 1) + (hp.far_items.empty() ? 0 : 1) +
+                            (hp.near_items.empty() ? 0 : 1) + 1 /* epilogue */;
     s->shared_batches = hp.shared_order ? 1 : 0;
     s->interp_degree = hp.degree;
     s->theta = hp.theta;
@@ -467,6 +465,9 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
     if (out_on_host) {
         BLTC_CUDA(h->out_stage.ensure((size_t)n_orb * N));
         d_out = h->out_stage.p;
+        // a sharded plan writes its own targets only: the caller's other elements must survive the copy back
+        if (hp.shard_world > 1)
+            BLTC_CUDA(cudaMemcpyAsync(d_out, out, (size_t)n_orb * N * sizeof(double), cudaMemcpyHostToDevice, st));
     }
 
     const size_t ns = hp.cluster_of_slot.size();
@@ -486,7 +487,6 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
     int o0 = 0;
     for (size_t g = 0; g < groups.size(); ++g) {
         const int ot = groups[g];
-        const int rv = targets_per_thread(ot) - 1;
         const KPar nk = kind == kYukawa ? make_kpar(k + o0, ot) : make_kpar_coulomb(sub ? alpha : 1.0);
         const EpiPar ep = kind == kYukawa ? make_epipar(k + o0, ot) : make_epipar_coulomb(sub ? alpha : 1.0);
         // exp underflow guard: not needed when k r < 700 for every pair (max_dist bounds r)
@@ -509,12 +509,12 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
                                 h->fhat.p, h->up_chunks.p, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
         // a3: far field
-        BLTC_CUDA(launch_far(kind, ot, sub, guard, h->far_items[rv].p, (int)hp.far_items[rv].size(), h->far_slots.p,
+        BLTC_CUDA(launch_far(kind, ot, sub, guard, h->far_items.p, (int)hp.far_items.size(), h->far_slots.p,
                              h->slot_nodes.p, h->what.p, h->fhat.p, hp.degree, h->tgt_rec, ftgt, nk,
                              h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[3], st));
         // a4: near field
-        BLTC_CUDA(launch_near(kind, ot, sub, guard, h->near_items[rv].p, (int)hp.near_items[rv].size(), h->near_ranges.p,
+        BLTC_CUDA(launch_near(kind, ot, sub, guard, h->near_items.p, (int)hp.near_items.size(), h->near_ranges.p,
                               h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
         // a5: epilogue
@@ -602,7 +602,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
     // work decomposition: pseudo-batches of 2048 targets, tiles of 8 groups inside them, and
     // nsplit equal source segments so that >= ~16 CTAs exist per resident CTA slot
     constexpr int64_t kPB = 2048;
-    std::vector<WorkItem> items[2];
+    std::vector<WorkItem> items;
     std::vector<Range> ranges;
     std::vector<int32_t> pb_begin, pb_count, pb_nseg;
     std::vector<int64_t> pb_base;
@@ -620,25 +620,23 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             pb_nseg.push_back(nsplit);
             pb_base.push_back((int64_t)nsplit * b0);
         }
-        for (int rv = 0; rv < 2; ++rv) {
-            const int unit = 32 << rv;
-            for (int64_t t0 = 0; t0 < M;) {
-                const int64_t pb = t0 / kPB, pb_end = std::min<int64_t>(M, (pb + 1) * kPB);
-                const int64_t groups = (pb_end - t0 + unit - 1) / unit;
-                int g = 8;
-                if (groups < 8) { g = 1; while (2 * g <= groups) g *= 2; }
-                int gs = 0; while ((1 << gs) < g) ++gs;
-                const int64_t cnt = std::min<int64_t>((int64_t)g * unit, pb_end - t0);
-                for (int s = 0; s < nsplit; ++s)
-                    items[rv].push_back(WorkItem{(int32_t)t0, (int32_t)cnt, gs, s, s + 1, 0,
-                                                 pb_base[pb] + (int64_t)s * pb_count[pb] + (t0 - pb * kPB)});
-                t0 += cnt;
-            }
+        const int unit = 32 * kTargetsPerThread;
+        for (int64_t t0 = 0; t0 < M;) {
+            const int64_t pb = t0 / kPB, pb_end = std::min<int64_t>(M, (pb + 1) * kPB);
+            const int64_t groups = (pb_end - t0 + unit - 1) / unit;
+            int g = 8;
+            if (groups < 8) { g = 1; while (2 * g <= groups) g *= 2; }
+            int gs = 0; while ((1 << gs) < g) ++gs;
+            const int64_t cnt = std::min<int64_t>((int64_t)g * unit, pb_end - t0);
+            for (int s = 0; s < nsplit; ++s)
+                items.push_back(WorkItem{(int32_t)t0, (int32_t)cnt, gs, s, s + 1, 0,
+                                         pb_base[pb] + (int64_t)s * pb_count[pb] + (t0 - pb * kPB)});
+            t0 += cnt;
         }
     }
     const int64_t partial_len = (int64_t)nsplit * M;
     const size_t npb = pb_begin.size();
-    TempBuf t_src_rec, t_tgt_rec, t_fsrc, t_ftgt, t_partial, t_items[2], t_ranges, t_pbb, t_pbc, t_pbn, t_pbs;
+    TempBuf t_src_rec, t_tgt_rec, t_fsrc, t_ftgt, t_partial, t_items, t_ranges, t_pbb, t_pbc, t_pbn, t_pbs;
     BLTC_CUDA(t_src_rec.alloc((size_t)N * sizeof(double4), st));
     BLTC_CUDA(t_tgt_rec.alloc((size_t)M * sizeof(double4), st));
     BLTC_CUDA(t_fsrc.alloc((size_t)N * kMaxOT * sizeof(double), st));
@@ -657,6 +655,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
     BLTC_CUDA(launch_pack_records(d_sr, d_w, nullptr, N, t_src_rec.as<double4>(), st));
     BLTC_CUDA(launch_pack_records(d_tg, nullptr, nullptr, M, t_tgt_rec.as<double4>(), st));
 
+    BLTC_CUDA(put(t_items, items.data(), items.size() * sizeof(WorkItem)));
     const std::vector<int> groups = orbital_groups(n_orb);
     if (g_direct_profiling) {
         for (auto& pr : g_direct_pairs) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -665,9 +664,6 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
     int o0 = 0;
     for (size_t g = 0; g < groups.size(); ++g) {
         const int ot = groups[g];
-        const int rv = targets_per_thread(ot) - 1;
-        if (!t_items[rv].p)
-            BLTC_CUDA(put(t_items[rv], items[rv].data(), items[rv].size() * sizeof(WorkItem)));
         const KPar nk = kind == kYukawa ? make_kpar(k + o0, ot) : make_kpar_coulomb(sub ? alpha : 1.0);
         const EpiPar ep = kind == kYukawa ? make_epipar(k + o0, ot) : make_epipar_coulomb(sub ? alpha : 1.0);
         BLTC_CUDA(launch_gather(d_fs, N, o0, ot, nullptr, N, t_fsrc.as<double>(), st));
@@ -677,7 +673,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
             BLTC_CUDA(cudaEventRecord(ea, st));
         }
-        BLTC_CUDA(launch_near(kind, ot, sub, true, t_items[rv].as<WorkItem>(), (int)items[rv].size(), t_ranges.as<Range>(),
+        BLTC_CUDA(launch_near(kind, ot, sub, true, t_items.as<WorkItem>(), (int)items.size(), t_ranges.as<Range>(),
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }

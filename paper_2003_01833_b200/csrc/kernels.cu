@@ -23,7 +23,13 @@
 namespace bltc {
 namespace {
 
-constexpr int kNearUnroll = 2, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
+#ifndef BLTC_NEAR_UNROLL
+#define BLTC_NEAR_UNROLL 2
+#endif
+#ifndef BLTC_FAR_UNROLL9
+#define BLTC_FAR_UNROLL9 9
+#endif
+constexpr int kNearUnroll = BLTC_NEAR_UNROLL, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
@@ -358,7 +364,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PD = ProxyRec<OT>::kDoubles;
     static_assert(kProxyTile * PD >= R * OT * 8 * 32, "reduction scratch fits in the tile");
-    constexpr int kU = N1 ? N1 : kFarUnroll;
+    constexpr int kU = N1 ? (N1 == 9 ? BLTC_FAR_UNROLL9 : N1) : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
@@ -607,7 +613,7 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
     return cudaGetLastError();
 }
 
-// kernel<R, OT, SUB, GUARD> dispatch on (ot, subtract, guard): R = 2 for ot <= 2, else 1
+// kernel<R, OT, SUB, GUARD> dispatch on (ot, subtract, guard); R = kTargetsPerThread = 2
 template <template <int, int, bool, bool> class K, typename... Args>
 cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int grid, cudaStream_t st, Args... args) {
 #define BLTC_GO(RV, OTV, SV, GV)                                                                        \
@@ -624,8 +630,8 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
     switch (ot) {
         case 1: BLTC_SG(2, 1)
         case 2: BLTC_SG(2, 2)
-        case 3: BLTC_SG(1, 3)
-        case 4: BLTC_SG(1, 4)
+        case 3: BLTC_SG(2, 3)
+        case 4: BLTC_SG(2, 4)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_SG

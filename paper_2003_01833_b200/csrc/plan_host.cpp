@@ -255,6 +255,13 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         for (int d = 0; d < 3; ++d) { p.b_lo[3 * b + d] = L.lo[d]; p.b_hi[3 * b + d] = L.hi[d]; }
     }
 
+    auto lap = [&, last = t0](int stage) mutable {
+        const auto now = std::chrono::steady_clock::now();
+        p.stage_ms[stage] += std::chrono::duration<double, std::milli>(now - last).count();
+        last = now;
+    };
+    lap(0);
+
     // line 3, decisions: per-batch interaction lists ("precomputed for each target batch").
     // Batches are independent: contiguous chunks of them are traversed by concurrent tasks into private
     // lists, concatenated in batch order (identical to the sequential result).
@@ -295,6 +302,8 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
             p.near_idx.insert(p.near_idx.end(), cnear[ch].begin(), cnear[ch].end());
         }
     }
+
+    lap(1);
 
     // batch slice of this rank: equal shares of the kernel evaluations (the batches are independent given
     // the sources and the proxy charges)
@@ -354,6 +363,8 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
             return (a.end - a.begin) > (c.end - c.begin);
         });
     }
+
+    lap(2);
 
     // ---- B200 work decomposition -------------------------------------------------------
     // Per batch: near clusters -> merged contiguous source ranges; far clusters -> slot ids.
@@ -434,19 +445,17 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         p.b_nseg_far[b] = (int32_t)fseg_slices.size();
         p.b_nseg_near[b] = (int32_t)nseg_slices.size();
         p.b_partial_base[b] = partial;
-        for (int rv = 0; rv < 2; ++rv) {
-            make_tiles(p.b_begin[b], p.b_end[b], 32 << rv, tiles, gsh);
-            for (size_t ti = 0; ti < tiles.size(); ++ti) {
-                const int64_t local = tiles[ti].first - p.b_begin[b];
-                for (size_t s = 0; s < fseg_slices.size(); ++s)
-                    p.far_items[rv].push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                        fseg_slices[s].first, fseg_slices[s].second, 0,
-                        partial + (int64_t)s * nt + local});
-                for (size_t s = 0; s < nseg_slices.size(); ++s)
-                    p.near_items[rv].push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                        nseg_slices[s].first, nseg_slices[s].second, 0,
-                        partial + (int64_t)(fseg_slices.size() + s) * nt + local});
-            }
+        make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh);
+        for (size_t ti = 0; ti < tiles.size(); ++ti) {
+            const int64_t local = tiles[ti].first - p.b_begin[b];
+            for (size_t s = 0; s < fseg_slices.size(); ++s)
+                p.far_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                    fseg_slices[s].first, fseg_slices[s].second, 0,
+                    partial + (int64_t)s * nt + local});
+            for (size_t s = 0; s < nseg_slices.size(); ++s)
+                p.near_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                    nseg_slices[s].first, nseg_slices[s].second, 0,
+                    partial + (int64_t)(fseg_slices.size() + s) * nt + local});
         }
         partial += (int64_t)(fseg_slices.size() + nseg_slices.size()) * nt;
     }
@@ -459,18 +468,19 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         return s << w.gshift;
     };
     auto far_cost_of = [&](const WorkItem& w) { return (int64_t)(w.list_end - w.list_begin) << w.gshift; };
-    for (int rv = 0; rv < 2; ++rv) {
-        std::vector<int64_t> key(p.near_items[rv].size());
-        for (size_t i = 0; i < key.size(); ++i) key[i] = near_cost_of(p.near_items[rv][i]);
+    {
+        std::vector<int64_t> key(p.near_items.size());
+        for (size_t i = 0; i < key.size(); ++i) key[i] = near_cost_of(p.near_items[i]);
         std::vector<size_t> ord(key.size());
         std::iota(ord.begin(), ord.end(), size_t(0));
         std::stable_sort(ord.begin(), ord.end(), [&](size_t a, size_t c) { return key[a] > key[c]; });
         std::vector<WorkItem> sorted(key.size());
-        for (size_t i = 0; i < ord.size(); ++i) sorted[i] = p.near_items[rv][ord[i]];
-        p.near_items[rv].swap(sorted);
-        std::stable_sort(p.far_items[rv].begin(), p.far_items[rv].end(),
+        for (size_t i = 0; i < ord.size(); ++i) sorted[i] = p.near_items[ord[i]];
+        p.near_items.swap(sorted);
+        std::stable_sort(p.far_items.begin(), p.far_items.end(),
                          [&](const WorkItem& a, const WorkItem& c) { return far_cost_of(a) > far_cost_of(c); });
     }
+    lap(3);
     p.build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
 }
 

@@ -24,7 +24,7 @@ struct Tree {
     std::vector<int> leaves;         // leaf ids in DFS order
 };
 
-// One CTA's work: a tile of targets (groups of 32*R consecutive targets; 2^gshift groups)
+// One CTA's work: a tile of targets (groups of 64 consecutive targets, 2 per thread; 2^gshift groups)
 // against one segment of its batch's far or near list.
 struct WorkItem {
     int32_t tgt_begin;               // first target (target tree order)
@@ -81,7 +81,7 @@ struct HostPlan {
     std::vector<int32_t> b_nseg_far, b_nseg_near;
     std::vector<int64_t> b_partial_base;       // per batch
     int64_t partial_len = 0;                   // doubles per orbital
-    std::vector<WorkItem> far_items[2], near_items[2];   // [0]: R = 1 (32 targets/group), [1]: R = 2
+    std::vector<WorkItem> far_items, near_items;   // target groups of 64 (2 targets per thread)
 
     // multi-GPU batch sharding: this plan carries the device work of the
     // batches [shard_b0, shard_b1) only -- a contiguous slice of the batch list holding ~1/world of the
@@ -92,6 +92,7 @@ struct HostPlan {
 
     double max_dist = 0;                       // upper bound of |target - source| over all pairs (root boxes)
     double build_ms = 0;
+    double stage_ms[4] = {0, 0, 0, 0};         // tree(s), MAC traversal, proxy slots + upward items, work decomposition
 };
 
 // Throws std::invalid_argument / std::bad_alloc.  targets == nullptr: targets are the sources.

@@ -35,28 +35,53 @@ class ShardExchange:
         self.counts = [int(v) for v in counts.cpu()]
         if sum(self.counts) != self.N:
             raise ValueError(f"shards cover {sum(self.counts)} of {self.N} targets")
-        self.cmax = max(self.counts)
-        pad = torch.zeros(self.cmax, dtype=torch.int64, device=device)
+        self.cmax = max(max(self.counts), 1)
+        pad = torch.zeros(self.cmax, dtype=torch.int64, device=device)       # padding reads column 0: harmless
         pad[: idx.numel()] = idx
-        gathered = [torch.empty_like(pad) for _ in range(self.world)]
-        dist.all_gather(gathered, pad, group=group)
-        self.idx = [g[: self.counts[r]] for r, g in enumerate(gathered)]      # every rank's targets
+        gathered = torch.empty(self.world * self.cmax, dtype=torch.int64, device=device)
+        dist.all_gather_into_tensor(gathered, pad, group=group)              # flat: rank r's block is [r*cmax, ...)
+        gathered = gathered.view(self.world, self.cmax)
+        self.idx = [gathered[r, : self.counts[r]] for r in range(self.world)]      # every rank's targets
         allidx = torch.cat(self.idx)
         if int(torch.unique(allidx).numel()) != self.N:
             raise ValueError("shards overlap")
         self.local_idx = idx
+        self._send_idx = pad
+        self._maps = {}                      # n_orb -> (positions in the gathered buffer, positions in out)
+
+    def _map(self, n_orb, device):
+        m = self._maps.get(n_orb)
+        if m is None:
+            torch = self.torch
+            src, dst = [], []
+            for r in range(self.world):
+                if r == self.rank or not self.counts[r]:
+                    continue
+                j = torch.arange(self.counts[r], dtype=torch.int64, device=device)
+                for o in range(n_orb):
+                    src.append((r * n_orb + o) * self.cmax + j)
+                    dst.append(o * self.N + self.idx[r])
+            e = torch.empty(0, dtype=torch.int64, device=device)
+            m = (torch.cat(src) if src else e, torch.cat(dst) if dst else e)
+            self._maps[n_orb] = m
+        return m
+
+    def bytes_per_step(self, n_orb):
+        """Bytes each rank receives per exchange: world x n_orb x cmax doubles (its own slice included)."""
+        return self.world * n_orb * self.cmax * 8
 
     def all_gather_out(self, out):
-        """out: [n_orb][N] tensor whose columns `local_idx` are valid on this rank; on return every column is."""
+        """out: contiguous [n_orb][N] tensor whose columns `local_idx` are valid on this rank; on return every
+        column is.  One gather kernel, ONE collective (all_gather_into_tensor of the ranks' padded slices), one
+        scatter kernel; the index maps are built once per n_orb."""
         torch, dist = self.torch, self.dist
         n_orb = out.shape[0]
-        send = torch.zeros((n_orb, self.cmax), dtype=out.dtype, device=out.device)
-        send[:, : self.counts[self.rank]] = out[:, self.local_idx]
-        recv = [torch.empty_like(send) for _ in range(self.world)]
-        dist.all_gather(recv, send, group=self.group)
-        for r in range(self.world):
-            if r != self.rank and self.counts[r]:
-                out[:, self.idx[r]] = recv[r][:, : self.counts[r]]
+        send = out.index_select(1, self._send_idx).view(-1)                     # [n_orb][cmax], flat
+        recv = torch.empty(self.world * n_orb * self.cmax, dtype=out.dtype, device=out.device)
+        dist.all_gather_into_tensor(recv, send, group=self.group)               # [world][n_orb][cmax], flat
+        src, dst = self._map(n_orb, out.device)
+        if src.numel():
+            out.view(-1).index_copy_(0, dst, recv.index_select(0, src))
         return out
 
 

@@ -40,10 +40,30 @@ def test_reference_arm_other_ranks_exit_quietly():
     assert r.returncode == 0 and r.stdout.strip() == ""
 
 
+def test_cpu_baseline_sample_uses_every_thread():
+    """The sampled oracle run is parallel over targets (not over the few sampled batches): its batch-sum phase scales
+    with OMP_NUM_THREADS, and `cores` is the thread count the library really uses."""
+    ncpu = os.cpu_count() or 1
+    if ncpu < 4:
+        pytest.skip("needs >= 4 cores")
+    code = ("import bench, json; c = bench.workload('cfg0'); v, dt, desc, cores = bench.cpu_oracle_sample(c, repeat=2); "
+            "print(json.dumps({'dt': dt, 'cores': cores, 'value': v}))")
+    res = {}
+    for nt in (1, 4):
+        env = dict(os.environ, OMP_NUM_THREADS=str(nt))
+        r = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=env, timeout=600, stdout=subprocess.PIPE,
+                           stderr=subprocess.PIPE, text=True)
+        assert r.returncode == 0, r.stderr[-2000:]
+        res[nt] = json.loads(r.stdout.strip().splitlines()[-1])
+        assert res[nt]["cores"] == nt
+    assert res[1]["dt"] / res[4]["dt"] > 2.0, res                # 4 threads: at least 2x faster than 1
+    assert res[4]["value"] / res[1]["value"] > 2.0, res
+
+
 @pytest.mark.gpu
 def test_cuda_arm_line_small_workload():
     d = _run("--workload", "cfg0", "--steps", "3", "--warmup", "3")
-    assert BASE_KEYS | {"roofline", "clocks", "phase_ms", "plan", "direct", "gi_update"} <= set(d)
+    assert BASE_KEYS | {"roofline", "clocks", "phase_ms", "plan", "direct", "gi_update", "cpu_baseline_fast"} <= set(d)
     assert "impl" not in d or d["impl"] != "reference"
     assert d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] >= 3 and d["dtype"] == "f64"
     rf = d["roofline"]
@@ -54,5 +74,9 @@ def test_cuda_arm_line_small_workload():
     assert e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == d["config"]["N"] * d["config"]["n_orb"] * 8
     assert e["value"] > 0 and e["value"] != d["value"] and e["bitwise_equal_to_device_path"] is True
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
+    assert d["cpu_baseline"]["cores"] == (os.cpu_count() if "OMP_NUM_THREADS" not in os.environ else int(os.environ["OMP_NUM_THREADS"]))
+    ref = _run("--impl", "reference", "--workload", "cfg0", "--steps", "2", "--warmup", "1")
+    assert ref["config"] == d["config"]                          # both arms describe the same workload
+    assert 0.5 < ref["value"] / d["cpu_baseline"]["value"] < 2.0
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(d["clocks"])
     assert abs(sum(d["phase_ms"].values()) - d["ms_per_step"]) < 0.2 * d["ms_per_step"]

@@ -110,7 +110,7 @@ def test_bench_flops_table_matches_the_built_sass():
             name = "c" + name
         key = (name, r["OT"])
         assert bench.FLOPS_PER_PAIR[key] == pytest.approx(r["flops"], abs=1e-9), (key, r)
-        assert r["R"] == (2 if r["OT"] <= 2 else 1)
+        assert r["R"] == 2
         seen.add(key)
     assert seen == set(bench.FLOPS_PER_PAIR)
 

@@ -175,7 +175,13 @@ def _check_tree(c, e, leaf_size):
         if e["cl_nchild"][i] == 0:
             covered[b:en] += 1
             ext = e["cl_hi"][i] - e["cl_lo"][i]
-            assert en - b <= leaf_size or ext.max() == 0.0 or True
+            # R4: a leaf holds <= N_L points, unless it cannot be cut (R5: all points coincide, or the box midpoint
+            # rounds onto a face so that every point falls into the same child)
+            if en - b > leaf_size and ext.max() > 0.0:
+                cut = (ext > 0) & (ext * np.sqrt(2.0) >= ext.max())
+                mid = 0.5 * (e["cl_lo"][i] + e["cl_hi"][i])
+                code = ((pts > mid) & cut) @ np.array([1, 2, 4])
+                assert len(np.unique(code)) == 1
         else:
             kids = np.nonzero(e["cl_parent"] == i)[0]
             assert len(kids) == e["cl_nchild"][i] and len(kids) in range(2, 9)

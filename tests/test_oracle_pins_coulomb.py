@@ -156,6 +156,26 @@ def test_coulomb_bltc_limits_error_trend_and_anchor(oracle_mod):
     assert 1e-8 < rel2(tc, ds) < 1e-4, rel2(tc, ds)
 
 
+def test_coulomb_far_field_loop_equals_the_pinned_far_field_loop_with_the_laplace_kernel(oracle_mod):
+    """oracle_bltc_eval_coulomb has its own far-field loop nest (bltc_cpu.c).  Its 1/r term must equal, sum for sum,
+    the far field of oracle_bltc_eval with the Laplace kernel 1/(4 pi r) (kind = 2) -- the loop nest whose indexing
+    is pinned exactly by the polynomial test kernel in test_oracle_pins.py -- and so must the near field."""
+    c = I.random_cloud(9000, seed=11, clustered=True, leaf_size=200, batch_size=200, degree=5)
+    P = (c.x, c.y, c.z)
+    pl = oracle_mod.OraclePlan(P, 0.7, 5, 200, 200)
+    assert pl.n_far > 200
+    f = c.f[0]
+    out_c, parts_c = pl.evaluate_coulomb(c.w, f, subtract=False, return_parts=True)
+    out_l, parts_l = pl.evaluate(c.w, f, 1.0, subtract=False, finalize=False, kind=2, return_parts=True)
+    far_c, near_c = parts_c
+    far_l, near_l = 4.0 * np.pi * parts_l[0], 4.0 * np.pi * parts_l[1]
+    assert np.abs(far_l).max() > 0
+    # term by term the two differ by one rounding (x / (4 pi r) * 4 pi  vs  x / r): 1e-15 per target
+    assert np.abs(far_c - far_l).max() <= 4e-15 * np.abs(far_l).max()
+    assert np.abs(near_c - near_l).max() <= 4e-15 * np.abs(near_l).max()
+    assert rel2(out_c, 4.0 * np.pi * out_l) < 1e-15
+
+
 def test_coulomb_bltc_rejects_bad_arguments(oracle_mod):
     c = I.random_cloud(300, seed=2, leaf_size=50, batch_size=50, degree=3)
     P = (c.x, c.y, c.z)

@@ -141,12 +141,14 @@ def _gloo_worker(rank, world, port, q):
         dist.destroy_process_group()
 
 
-def test_world2_gloo_sharded_convolution_assembles_to_the_full_result(oracle_mod):
+@pytest.mark.parametrize("world", [2, 4])
+def test_gloo_sharded_convolution_assembles_to_the_full_result(oracle_mod, world):
+    # world 4 on this cloud's batches leaves uneven slices; test_gloo_exchange_with_an_empty_slice covers an empty one
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_gloo_worker, args=(r, world, port, q)) for r in range(world)]
     for p in procs:
         p.start()
     res = q.get(timeout=300)
@@ -154,6 +156,68 @@ def test_world2_gloo_sharded_convolution_assembles_to_the_full_result(oracle_mod
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res == (True, True, True), res
+
+
+def _gloo_empty_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2003_01833_b200.multi_gpu import ShardExchange
+        # 3 batches over 4 ranks: at least one rank owns nothing (bltc_create_sharded gives it an empty slice)
+        c = I.random_cloud(150, seed=3, leaf_size=200, batch_size=200, degree=3)   # one batch: three ranks own nothing
+        p = B.bltc_create_host_plan_sharded(None, c.coords(), None, c.N, 0.5, 3, 200, 200, rank, world)
+        idx = B.bltc_get_shard_targets(p)
+        ex = ShardExchange(idx, c.N, "cpu")
+        out = torch.full((3, c.N), float("nan"), dtype=torch.float64)
+        col = torch.from_numpy(idx)
+        out[:, col] = torch.arange(3, dtype=torch.float64)[:, None] * 1000.0 + col.to(torch.float64)[None, :]
+        ex.all_gather_out(out)
+        want = torch.arange(3, dtype=torch.float64)[:, None] * 1000.0 + torch.arange(c.N, dtype=torch.float64)[None, :]
+        n_empty = torch.tensor([int(len(idx) == 0)])
+        dist.all_reduce(n_empty)
+        ok = torch.tensor([int(torch.equal(out, want))])
+        dist.all_reduce(ok)
+        if rank == 0:
+            q.put((int(ok.item()), int(n_empty.item()), ex.bytes_per_step(3)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_gloo_exchange_with_an_empty_slice():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gloo_empty_worker, args=(r, 4, port, q)) for r in range(4)]
+    for p in procs:
+        p.start()
+    ok, n_empty, nbytes = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert ok == 4 and n_empty >= 1 and nbytes > 0
+
+
+@pytest.mark.gpu
+def test_gpu_sharded_plan_host_out_keeps_the_other_ranks_elements():
+    # bltc.h: a sharded plan writes its own targets only -- also when `out` is a host buffer staged through the device
+    import torch
+    c = _cloud()
+    X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+    plan = B.bltc_create_sharded(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, 1, 3)
+    idx = B.bltc_get_shard_targets(plan)
+    dev = torch.full((c.n_orb, c.N), float("nan"), dtype=torch.float64, device="cuda")
+    B.bltc_convolve(plan, c.k, f, c.n_orb, dev, True)
+    host = np.full((c.n_orb, c.N), np.nan)
+    B.bltc_convolve(plan, c.k, f, c.n_orb, host, True)
+    torch.cuda.synchronize()
+    mine = np.zeros(c.N, bool); mine[idx] = True
+    assert np.isnan(host[:, ~mine]).all() and not np.isnan(host[:, mine]).any()
+    np.testing.assert_array_equal(host[:, mine], dev.cpu().numpy()[:, mine])
+    B.bltc_destroy(plan)
 
 
 @pytest.mark.gpu
