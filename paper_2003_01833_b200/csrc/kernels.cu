@@ -23,13 +23,7 @@
 namespace bltc {
 namespace {
 
-#ifndef BLTC_NEAR_UNROLL
-#define BLTC_NEAR_UNROLL 2
-#endif
-#ifndef BLTC_FAR_UNROLL9
-#define BLTC_FAR_UNROLL9 9
-#endif
-constexpr int kNearUnroll = BLTC_NEAR_UNROLL, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
+constexpr int kNearUnroll = 2, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
@@ -364,7 +358,7 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PD = ProxyRec<OT>::kDoubles;
     static_assert(kProxyTile * PD >= R * OT * 8 * 32, "reduction scratch fits in the tile");
-    constexpr int kU = N1 ? (N1 == 9 ? BLTC_FAR_UNROLL9 : N1) : kFarUnroll;
+    constexpr int kU = N1 ? N1 : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
