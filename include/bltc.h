@@ -30,8 +30,12 @@
  *   - The library copies what it needs: inputs of bltc_create may be freed after it returns;
  *     f/out of a convolve call must stay valid until the stream has executed the call.
  *   - Return value: 0 on success, a negative bltc_status otherwise; bltc_last_error() gives a
- *     thread-local message.  No exceptions, no exit(), no global state; handles are independent.
- *     A handle must not be used by two threads at once.
+ *     thread-local message.  No exceptions, no exit(); handles are independent and the library keeps no state
+ *     between calls other than a stream-ordered memory pool of its own per device (staging buffers of
+ *     direct_convolve / bltc_gi_update are reused, the device's default pool is not touched).
+ *     A handle must not be used by two threads at once, and calls on one handle must be stream-ordered with
+ *     respect to each other (the per-plan scratch -- proxy charges, partial sums, staging -- is shared by them):
+ *     use one stream per handle, or make the second stream wait on the first.
  *   - There is no CPU fallback: every compute entry point fails with BLTC_ECUDA / BLTC_ENODEVICE
  *     if no CUDA device is usable.
  *   - Limits: 1 <= N <= 2e9 (int32 indices), 1 <= interp_degree <= 20, 0 <= theta < 1,
@@ -78,7 +82,7 @@ typedef struct bltc_stats {
     int32_t shared_batches;    /* 1: batches are the source leaves */
     int32_t interp_degree;
     double  theta;
-    double  build_ms;          /* host wall-clock of tree + lists + work decomposition */
+    double  build_ms;          /* wall-clock of tree + lists + work decomposition (device builder: kernels included) */
     double  upload_ms;         /* host wall-clock of device upload + f-independent proxy weights */
     /* batch sharding (bltc_create_sharded); an unsharded plan reports rank 0 of 1 and all batches */
     int32_t shard_rank, shard_world;
@@ -87,6 +91,13 @@ typedef struct bltc_stats {
     int64_t shard_targets;     /* ... = this many targets (a contiguous range in target tree order) */
     int64_t shard_far_evals;   /* kernel evaluations per orbital of this plan's batches */
     int64_t shard_near_evals;
+    /* step a0 timing (host wall-clock, ms; the kernels of the device builder are synchronised inside) */
+    double  tree_ms;           /* cluster tree(s) + batches */
+    double  lists_ms;          /* MAC traversal of Algorithm 3 (decisions) */
+    double  decomp_ms;         /* proxy slots, Chebyshev grids, work decomposition */
+    double  create_ms;         /* all of bltc_create, uploads and the proxy weights of w included */
+    int32_t built_on_device;   /* 1: tree and lists were built by kernels (BLTC_BUILDER_DEVICE) */
+    int32_t reserved;
 } bltc_stats;
 
 /* Phases of one bltc_convolve, for bltc_get_phase_ms (device times, CUDA events on `stream`). */
@@ -101,8 +112,12 @@ enum { BLTC_PHASE_GATHER = 0, BLTC_PHASE_UPWARD = 1, BLTC_PHASE_FAR = 2, BLTC_PH
  *   theta, interp_degree: MAC parameter and degree n of Eq. (36).
  *   batch_size N_B, leaf_size N_L: PAPER.md:378,428.  If N_B == N_L and targets are the sources the
  *   batches are the leaf clusters.
- * Builds the tree, batches, lists on the host, uploads tree-ordered data and computes the proxy
- * weights of w (what_k).  Synchronous.  *h is set only on success.
+ * Builds the tree, batches and lists ON THE DEVICE (SURVEY.md 8(f) NEXT-4a; the precompute stage is
+ * what limits the paper's multi-GPU scaling): per tree level exact min/max boxes, the split decisions of DESIGN.md
+ * readings R4-R5, one stable radix sort of (segment, child code) keys; one thread per batch walks the tree for the
+ * MAC lists.  The plan is identical -- cluster for cluster, list entry for list entry -- to the host builder's and
+ * to the CPU oracle's.  Then uploads the work decomposition and computes the proxy weights of w (what_k).
+ * Inputs on the device are used in place (no copy to the host).  Synchronous.  *h is set only on success.
  */
 int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                 int64_t N, double theta, int interp_degree, int batch_size, int leaf_size);
@@ -121,6 +136,13 @@ int bltc_create(bltc_handle* h, const double* targets, const double* sources, co
 int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                         int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
                         int rank, int world);
+/* The same with the builder named: BLTC_BUILDER_DEVICE (what bltc_create / bltc_create_sharded use) or
+ * BLTC_BUILDER_HOST (tree, lists and decomposition by the threaded host code of plan_host.cpp -- the setup
+ * alternative; also taken automatically for N >= 2^28).  Both give the same plan. */
+enum { BLTC_BUILDER_DEVICE = 0, BLTC_BUILDER_HOST = 1 };
+int bltc_create_with_builder(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                             int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
+                             int rank, int world, int builder);
 int bltc_create_host_plan_sharded(bltc_handle* h, const double* targets, const double* sources,
                                   const double* weights, int64_t N, double theta, int interp_degree,
                                   int batch_size, int leaf_size, int rank, int world);
@@ -151,6 +173,10 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
  *   targets double[3][M], f_targets double[n_orb][M] (may be NULL iff subtract_singularity == 0),
  *   sources double[3][N], weights double[N], f_sources double[n_orb][N], k HOST double[n_orb],
  *   out double[n_orb][M].
+ * The call synchronises `stream` once before the pair kernel is enqueued: the bounding boxes of target and
+ * source chunks are read back to choose the kernel variant (r == 0 test only where a source chunk can meet a
+ * target chunk, exp underflow guard only if k_max x the largest distance can reach 700).  Its profiling switch
+ * (bltc_direct_set_profiling) is per calling thread.
  */
 int direct_convolve(const double* targets, const double* f_targets, int64_t M,
                     const double* sources, const double* weights, const double* f_sources, int64_t N,

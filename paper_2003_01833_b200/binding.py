@@ -36,10 +36,13 @@ class bltc_stats(C.Structure):
         ("shared_batches", C.c_int32), ("interp_degree", C.c_int32),
         ("theta", C.c_double), ("build_ms", C.c_double), ("upload_ms", C.c_double),
         ("shard_rank", C.c_int32), ("shard_world", C.c_int32)] + [(n, C.c_int64) for n in (
-            "shard_batch_begin", "shard_batch_end", "shard_targets", "shard_far_evals", "shard_near_evals")]
+            "shard_batch_begin", "shard_batch_end", "shard_targets", "shard_far_evals", "shard_near_evals")] + [
+        ("tree_ms", C.c_double), ("lists_ms", C.c_double), ("decomp_ms", C.c_double), ("create_ms", C.c_double),
+        ("built_on_device", C.c_int32), ("reserved", C.c_int32)]
 
 
 EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
+            "bltc_create_with_builder",
             "bltc_get_shard_targets", "bltc_convolve", "direct_convolve",
             "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
@@ -63,6 +66,7 @@ def lib():
     L.bltc_create_host_plan.argtypes = L.bltc_create.argtypes
     L.bltc_create_sharded.argtypes = L.bltc_create.argtypes + [C.c_int, C.c_int]
     L.bltc_create_host_plan_sharded.argtypes = L.bltc_create_sharded.argtypes
+    L.bltc_create_with_builder.argtypes = L.bltc_create_sharded.argtypes + [C.c_int]
     L.bltc_get_shard_targets.argtypes = [vp, _i64p]
     L.bltc_convolve.argtypes = [vp, _dp, vp, C.c_int, vp, C.c_int, vp]
     L.direct_convolve.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, _dp, C.c_int, vp, C.c_int, vp]
@@ -93,8 +97,10 @@ def _check(rc):
         raise BltcError(rc, lib().bltc_last_error().decode())
 
 
-def _ptr(a, what, allow_none=False):
-    """Raw address of a float64 contiguous torch tensor / numpy array (keeps no reference)."""
+def _ptr(a, what, allow_none=False, count=None):
+    """Raw address of a float64 contiguous torch tensor / numpy array (keeps no reference).  count: the number of
+    doubles the library will read or write there -- a smaller buffer is a ValueError here, not an out-of-bounds
+    access inside a kernel."""
     if a is None:
         if allow_none:
             return None
@@ -102,11 +108,15 @@ def _ptr(a, what, allow_none=False):
     if isinstance(a, np.ndarray):
         if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"]:
             raise ValueError(f"{what}: need a C-contiguous float64 array")
+        if count is not None and a.size < count:
+            raise ValueError(f"{what}: need at least {count} elements, got {a.size}")
         return a.ctypes.data
     import torch
     if isinstance(a, torch.Tensor):
         if a.dtype != torch.float64 or not a.is_contiguous():
             raise ValueError(f"{what}: need a contiguous float64 tensor")
+        if count is not None and a.numel() < count:
+            raise ValueError(f"{what}: need at least {count} elements, got {a.numel()}")
         return a.data_ptr()
     raise TypeError(f"{what}: expected numpy array or torch tensor")
 
@@ -150,8 +160,8 @@ class Plan:
 
 def _create(fn, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, *shard):
     h = C.c_void_p()
-    _check(fn(C.byref(h), _ptr(targets, "targets", True), _ptr(sources, "sources"),
-              _ptr(weights, "weights", True), int(N), float(theta), int(interp_degree),
+    _check(fn(C.byref(h), _ptr(targets, "targets", True, 3 * int(N)), _ptr(sources, "sources", False, 3 * int(N)),
+              _ptr(weights, "weights", True, int(N)), int(N), float(theta), int(interp_degree),
               int(batch_size), int(leaf_size), *[int(v) for v in shard]))
     return Plan(h, int(N))
 
@@ -181,6 +191,17 @@ def bltc_create(targets, sources, weights, N, theta, interp_degree, batch_size, 
     return _create(lib().bltc_create, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size)
 
 
+BUILDER_DEVICE, BUILDER_HOST = 0, 1
+
+
+def bltc_create_with_builder(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size,
+                             rank=0, world=1, builder=BUILDER_DEVICE):
+    """include/bltc.h bltc_create_with_builder: tree and lists by kernels (BUILDER_DEVICE, what bltc_create uses)
+    or by the threaded host code (BUILDER_HOST); both give the same plan."""
+    return _create(lib().bltc_create_with_builder, targets, sources, weights, N, theta, interp_degree, batch_size,
+                   leaf_size, rank, world, builder)
+
+
 def bltc_create_host_plan(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size):
     return _create(lib().bltc_create_host_plan, targets, sources, weights, N, theta, interp_degree,
                    batch_size, leaf_size)
@@ -189,7 +210,8 @@ def bltc_create_host_plan(targets, sources, weights, N, theta, interp_degree, ba
 def bltc_convolve(plan, k, f, n_orb, out, subtract_singularity=True, stream=None):
     """include/bltc.h bltc_convolve.  f, out: [n_orb][N] device or host buffers."""
     kk = _karray(k, n_orb)
-    _check(lib().bltc_convolve(plan._h, kk.ctypes.data_as(_dp), _ptr(f, "f"), int(n_orb), _ptr(out, "out"),
+    n = int(n_orb) * plan.N
+    _check(lib().bltc_convolve(plan._h, kk.ctypes.data_as(_dp), _ptr(f, "f", False, n), int(n_orb), _ptr(out, "out", False, n),
                                int(bool(subtract_singularity)), _stream_ptr(stream)))
     return out
 
@@ -198,16 +220,18 @@ def direct_convolve(targets, f_targets, M, sources, weights, f_sources, N, k, n_
                     subtract_singularity=True, stream=None):
     """include/bltc.h direct_convolve."""
     kk = _karray(k, n_orb)
-    _check(lib().direct_convolve(_ptr(targets, "targets"), _ptr(f_targets, "f_targets", True), int(M),
-                                 _ptr(sources, "sources"), _ptr(weights, "weights"),
-                                 _ptr(f_sources, "f_sources"), int(N), kk.ctypes.data_as(_dp), int(n_orb),
-                                 _ptr(out, "out"), int(bool(subtract_singularity)), _stream_ptr(stream)))
+    M, N, n_orb = int(M), int(N), int(n_orb)
+    _check(lib().direct_convolve(_ptr(targets, "targets", False, 3 * M), _ptr(f_targets, "f_targets", True, n_orb * M), M,
+                                 _ptr(sources, "sources", False, 3 * N), _ptr(weights, "weights", False, N),
+                                 _ptr(f_sources, "f_sources", False, n_orb * N), N, kk.ctypes.data_as(_dp), n_orb,
+                                 _ptr(out, "out", False, n_orb * M), int(bool(subtract_singularity)), _stream_ptr(stream)))
     return out
 
 
 def bltc_convolve_coulomb(plan, f, n_f, out, subtract_singularity=True, alpha=1.0, stream=None):
     """include/bltc.h bltc_convolve_coulomb (Hartree potential, Gaussian singularity subtraction)."""
-    _check(lib().bltc_convolve_coulomb(plan._h, _ptr(f, "f"), int(n_f), _ptr(out, "out"),
+    n = int(n_f) * plan.N
+    _check(lib().bltc_convolve_coulomb(plan._h, _ptr(f, "f", False, n), int(n_f), _ptr(out, "out", False, n),
                                        int(bool(subtract_singularity)), float(alpha), _stream_ptr(stream)))
     return out
 
@@ -215,9 +239,10 @@ def bltc_convolve_coulomb(plan, f, n_f, out, subtract_singularity=True, alpha=1.
 def direct_convolve_coulomb(targets, f_targets, M, sources, weights, f_sources, N, n_f, out,
                             subtract_singularity=True, alpha=1.0, stream=None):
     """include/bltc.h direct_convolve_coulomb."""
-    _check(lib().direct_convolve_coulomb(_ptr(targets, "targets"), _ptr(f_targets, "f_targets", True), int(M),
-                                         _ptr(sources, "sources"), _ptr(weights, "weights"),
-                                         _ptr(f_sources, "f_sources"), int(N), int(n_f), _ptr(out, "out"),
+    M, N, n_f = int(M), int(N), int(n_f)
+    _check(lib().direct_convolve_coulomb(_ptr(targets, "targets", False, 3 * M), _ptr(f_targets, "f_targets", True, n_f * M), M,
+                                         _ptr(sources, "sources", False, 3 * N), _ptr(weights, "weights", False, N),
+                                         _ptr(f_sources, "f_sources", False, n_f * N), N, n_f, _ptr(out, "out", False, n_f * M),
                                          int(bool(subtract_singularity)), float(alpha), _stream_ptr(stream)))
     return out
 
@@ -225,9 +250,10 @@ def direct_convolve_coulomb(targets, f_targets, M, sources, weights, f_sources, 
 def bltc_gi_update(w, psi_old, f_old, psi_new, phi, n_prev, N, eps_old, result, stream=None):
     """include/bltc.h bltc_gi_update (Green Iteration, Alg. 2 lines 4-7).  psi_new is updated in place;
     result: float64[4 + n_prev] buffer (device or host) = eps_new, delta, norm, residual, coefficients."""
-    _check(lib().bltc_gi_update(_ptr(w, "w"), _ptr(psi_old, "psi_old"), _ptr(f_old, "f_old"),
-                                _ptr(psi_new, "psi_new"), _ptr(phi, "phi", True), int(n_prev), int(N),
-                                float(eps_old), _ptr(result, "result"), _stream_ptr(stream)))
+    N, n_prev = int(N), int(n_prev)
+    _check(lib().bltc_gi_update(_ptr(w, "w", False, N), _ptr(psi_old, "psi_old", False, N), _ptr(f_old, "f_old", False, N),
+                                _ptr(psi_new, "psi_new", False, N), _ptr(phi, "phi", True, n_prev * N), n_prev, N,
+                                float(eps_old), _ptr(result, "result", False, 4 + n_prev), _stream_ptr(stream)))
     return result
 
 

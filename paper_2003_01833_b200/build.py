@@ -8,8 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbltc.so")
-SOURCES = ["api.cu", "kernels.cu", "gi_kernels.cu", "plan_host.cpp"]
-HEADERS = ["kernels.cuh", "gi_kernels.cuh", "fp64_math.cuh", "plan_host.hpp", os.path.join("..", "..", "include", "bltc.h")]
+SOURCES = ["api.cu", "kernels.cu", "gi_kernels.cu", "plan_device.cu", "plan_host.cpp"]
+HEADERS = ["kernels.cuh", "gi_kernels.cuh", "fp64_math.cuh", "plan_host.hpp", "plan_device.cuh", "exp_table.inc", os.path.join("..", "..", "include", "bltc.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall,-pthread",

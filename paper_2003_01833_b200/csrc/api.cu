@@ -7,6 +7,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <stdexcept>
 #include <string>
@@ -15,6 +16,7 @@
 #include "../../include/bltc.h"
 #include "gi_kernels.cuh"
 #include "kernels.cuh"
+#include "plan_device.cuh"
 #include "plan_host.hpp"
 
 using namespace bltc;
@@ -69,23 +71,34 @@ struct TempBuf {
     ~TempBuf() { if (p) cudaFreeAsync(p, st); }
     cudaError_t alloc(size_t bytes, cudaStream_t s) {
         st = s;
-        keep_pool_memory();
-        return cudaMallocAsync(&p, bytes ? bytes : 1, s);
+        cudaMemPool_t pool = library_pool();
+        if (!pool) return cudaMallocAsync(&p, bytes ? bytes : 1, s);
+        return cudaMallocFromPoolAsync(&p, bytes ? bytes : 1, pool, s);
     }
-    // The default memory pool hands its memory back to the driver at every synchronisation unless a release
-    // threshold is set; a call that stages a few buffers would then pay a real cudaMalloc/cudaFree (~ms) each
-    // time.  Set once per device: freed blocks stay in the pool for the next call.
-    static void keep_pool_memory() {
-        static bool done[64] = {};
+    // The library's OWN stream-ordered pool, one per device, created on first use and kept for the life of the
+    // process.  Its release threshold is unlimited, so the staging buffers of one call are reused by the next
+    // instead of going back to the driver at every synchronisation (a real cudaMalloc/cudaFree, ~ms per call);
+    // the device's default pool -- the caller's -- is left as it is.
+    static cudaMemPool_t library_pool() {
+        static std::mutex mu;
+        static cudaMemPool_t pools[64] = {};
         int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || done[dev]) return;
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return nullptr; }
+        std::lock_guard<std::mutex> lock(mu);
+        if (!pools[dev]) {
+            cudaMemPoolProps props = {};
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = dev;
+            cudaMemPool_t pool = nullptr;
+            if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
             unsigned long long keep = ~0ull;
             cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            cudaGetLastError();
+            pools[dev] = pool;
         }
-        cudaGetLastError();
-        done[dev] = true;
+        return pools[dev];
     }
     template <typename T> T* as() const { return static_cast<T*>(p); }
 };
@@ -108,8 +121,9 @@ std::vector<int> orbital_groups(int n_orb) {
     return g;
 }
 
-bool g_direct_profiling = false;
-std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_direct_pairs;
+// direct_convolve has no handle to carry its profiling switch and events: they are per calling thread
+thread_local bool g_direct_profiling = false;
+thread_local std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_direct_pairs;
 
 }  // namespace
 
@@ -117,13 +131,13 @@ struct bltc_plan_s {
     HostPlan hp;
     bool on_device = false;
     int device = 0;
-    double upload_ms = 0;
+    double upload_ms = 0, create_ms = 0;
     // static device state
     DevBuf<double4> src_rec, tgt_rec_own;
     const double4* tgt_rec = nullptr;
     DevBuf<int32_t> src_perm, tgt_perm_own;
     const int32_t* tgt_perm = nullptr;
-    DevBuf<int32_t> b_begin, b_count, b_nseg, slot_begin, slot_end, far_slots;
+    DevBuf<int32_t> b_begin, b_count, b_nseg, far_slots;
     DevBuf<int64_t> b_partial_base;
     DevBuf<double> slot_nodes, what;
     DevBuf<Range> near_ranges;
@@ -166,6 +180,23 @@ int build_plan_guarded(bltc_plan_s* pl, const double* targets, const double* sou
     return BLTC_OK;
 }
 
+// A device-built plan keeps its permutations on the device only; the host copies are made on first use.
+cudaError_t ensure_host_perm(bltc_plan_s* h) {
+    HostPlan& hp = h->hp;
+    auto fetch = [&](std::vector<int64_t>& dst, const int32_t* src) -> cudaError_t {
+        if (!dst.empty() || !src) return cudaSuccess;
+        std::vector<int32_t> tmp((size_t)hp.N);
+        cudaError_t e = cudaMemcpy(tmp.data(), src, tmp.size() * sizeof(int32_t), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return e;
+        dst.assign(tmp.begin(), tmp.end());
+        return cudaSuccess;
+    };
+    if (!h->on_device) return cudaSuccess;
+    cudaError_t e = fetch(hp.src.perm, h->src_perm.p);
+    if (e == cudaSuccess && !hp.shared_order) e = fetch(hp.tgt.perm, h->tgt_perm_own.p);
+    return e;
+}
+
 std::vector<int32_t> to_i32(const std::vector<int64_t>& v) {
     std::vector<int32_t> o(v.size());
     for (size_t i = 0; i < v.size(); ++i) o[i] = (int32_t)v[i];
@@ -203,39 +234,35 @@ int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* s
 
 int bltc_create(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                 int64_t N, double theta, int interp_degree, int batch_size, int leaf_size) {
-    return bltc_create_sharded(h, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, 0, 1);
+    return bltc_create_with_builder(h, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, 0, 1,
+                                    BLTC_BUILDER_DEVICE);
 }
 
 int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                         int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
                         int rank, int world) {
+    return bltc_create_with_builder(h, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, rank,
+                                    world, BLTC_BUILDER_DEVICE);
+}
+
+int bltc_create_with_builder(bltc_handle* h, const double* targets, const double* sources, const double* weights,
+                             int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
+                             int rank, int world, int builder) {
     int rc = check_create_args(h, sources, N, theta, interp_degree, batch_size, leaf_size);
     if (rc) return rc;
     if (world < 1 || rank < 0 || rank >= world) return fail(BLTC_EINVAL, "need 0 <= rank < world");
     if (!weights) return fail(BLTC_EINVAL, "weights is NULL");
+    if (builder != BLTC_BUILDER_DEVICE && builder != BLTC_BUILDER_HOST) return fail(BLTC_EINVAL, "unknown builder");
+    if (N >= ((int64_t)1 << 28)) builder = BLTC_BUILDER_HOST;     // the device builder's sort keys are 32-bit
     int dev = 0, sms = 0;
     BLTC_CUDA(cudaGetDevice(&dev));
     BLTC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-
-    // host copies of the coordinates (the tree is built on the host, timed separately)
+    const auto t_begin = std::chrono::steady_clock::now();
     const bool same = (targets == nullptr || targets == sources);
-    std::vector<double> hs, ht, hw;
-    try {
-        hs.resize(3 * (size_t)N); hw.resize((size_t)N);
-        if (!same) ht.resize(3 * (size_t)N);
-    } catch (const std::bad_alloc&) { return fail(BLTC_ENOMEM, "host allocation failed"); }
-    BLTC_CUDA(cudaMemcpy(hs.data(), sources, hs.size() * sizeof(double), cudaMemcpyDefault));
-    BLTC_CUDA(cudaMemcpy(hw.data(), weights, hw.size() * sizeof(double), cudaMemcpyDefault));
-    if (!same) BLTC_CUDA(cudaMemcpy(ht.data(), targets, ht.size() * sizeof(double), cudaMemcpyDefault));
 
     bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
     if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
-    rc = build_plan_guarded(pl, same ? nullptr : ht.data(), hs.data(), N, theta, interp_degree,
-                            batch_size, leaf_size, sms, rank, world);
-    if (rc) { delete pl; return rc; }
     pl->device = dev;
-
-    const auto t0 = std::chrono::steady_clock::now();
     HostPlan& hp = pl->hp;
 #define BLTC_TRY_OR_FREE(call)                                                                 \
     do {                                                                                       \
@@ -246,24 +273,82 @@ int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sou
                         std::string(#call) + ": " + cudaGetErrorString(e__));                  \
         }                                                                                      \
     } while (0)
-    // tree-ordered records
-    {
-        DevBuf<double> d_coords, d_w;
-        BLTC_TRY_OR_FREE(d_coords.upload(hs));
-        BLTC_TRY_OR_FREE(d_w.upload(hw));
+
+    // device views of the inputs (host arrays are uploaded once; device arrays are used in place)
+    DevBuf<double> up_src, up_tgt, up_w;
+    const double *d_src = sources, *d_tgt = same ? sources : targets, *d_w = weights;
+    if (!is_device_ptr(sources)) {
+        BLTC_TRY_OR_FREE(up_src.ensure(3 * (size_t)N));
+        BLTC_TRY_OR_FREE(cudaMemcpy(up_src.p, sources, 3 * (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
+        d_src = up_src.p;
+        if (same) d_tgt = d_src;
+    }
+    if (!same && !is_device_ptr(targets)) {
+        BLTC_TRY_OR_FREE(up_tgt.ensure(3 * (size_t)N));
+        BLTC_TRY_OR_FREE(cudaMemcpy(up_tgt.p, targets, 3 * (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
+        d_tgt = up_tgt.p;
+    }
+    if (!is_device_ptr(weights)) {
+        BLTC_TRY_OR_FREE(up_w.ensure((size_t)N));
+        BLTC_TRY_OR_FREE(cudaMemcpy(up_w.p, weights, (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
+        d_w = up_w.p;
+    }
+
+    if (builder == BLTC_BUILDER_HOST) {
+        // the host builder needs host copies of the coordinates
+        std::vector<double> hs, ht;
+        try {
+            hs.resize(3 * (size_t)N);
+            if (!same) ht.resize(3 * (size_t)N);
+        } catch (const std::bad_alloc&) { delete pl; return fail(BLTC_ENOMEM, "host allocation failed"); }
+        BLTC_TRY_OR_FREE(cudaMemcpy(hs.data(), sources, hs.size() * sizeof(double), cudaMemcpyDefault));
+        if (!same) BLTC_TRY_OR_FREE(cudaMemcpy(ht.data(), targets, ht.size() * sizeof(double), cudaMemcpyDefault));
+        rc = build_plan_guarded(pl, same ? nullptr : ht.data(), hs.data(), N, theta, interp_degree,
+                                batch_size, leaf_size, sms, rank, world);
+        if (rc) { delete pl; return rc; }
         BLTC_TRY_OR_FREE(pl->src_perm.upload(to_i32(hp.src.perm)));
-        BLTC_TRY_OR_FREE(pl->src_rec.ensure((size_t)N));
-        BLTC_TRY_OR_FREE(launch_pack_records(d_coords.p, d_w.p, pl->src_perm.p, N, pl->src_rec.p, nullptr));
-        if (hp.shared_order) {
-            pl->tgt_rec = pl->src_rec.p; pl->tgt_perm = pl->src_perm.p;
-        } else {
-            if (!same) BLTC_TRY_OR_FREE(d_coords.upload(ht));
-            BLTC_TRY_OR_FREE(pl->tgt_perm_own.upload(to_i32(hp.tgt.perm)));
-            BLTC_TRY_OR_FREE(pl->tgt_rec_own.ensure((size_t)N));
-            BLTC_TRY_OR_FREE(launch_pack_records(d_coords.p, nullptr, pl->tgt_perm_own.p, N, pl->tgt_rec_own.p, nullptr));
-            pl->tgt_rec = pl->tgt_rec_own.p; pl->tgt_perm = pl->tgt_perm_own.p;
+        if (!hp.shared_order) BLTC_TRY_OR_FREE(pl->tgt_perm_own.upload(to_i32(hp.tgt.perm)));
+    } else {
+        // NEXT-4a: tree(s) and MAC lists by kernels (plan_device.cu); decisions identical to the host builder's
+        const auto t0 = std::chrono::steady_clock::now();
+        auto ms_since = [](std::chrono::steady_clock::time_point a) {
+            return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - a).count();
+        };
+        try {
+            plan_begin(hp, N, same, theta, interp_degree, batch_size, leaf_size);
+            hp.built_on_device = true;
+            BLTC_TRY_OR_FREE(pl->src_perm.ensure((size_t)N));
+            BLTC_TRY_OR_FREE(build_tree_device(hp.src, d_src, N, leaf_size, pl->src_perm.p, nullptr));
+            if (!hp.shared_order) {
+                BLTC_TRY_OR_FREE(pl->tgt_perm_own.ensure((size_t)N));
+                BLTC_TRY_OR_FREE(build_tree_device(hp.tgt, d_tgt, N, batch_size, pl->tgt_perm_own.p, nullptr));
+            }
+            plan_set_batches(hp);
+            hp.stage_ms[0] = ms_since(t0);
+            const auto t1 = std::chrono::steady_clock::now();
+            BLTC_TRY_OR_FREE(build_lists_device(hp, rank, world, nullptr));
+            hp.stage_ms[1] = ms_since(t1);
+            const auto t2 = std::chrono::steady_clock::now();
+            plan_finish(hp, sms);
+            hp.stage_ms[3] = ms_since(t2);
+        } catch (const std::bad_alloc&) {
+            delete pl; return fail(BLTC_ENOMEM, "host allocation failed while building the plan");
+        } catch (const std::exception& e) {
+            delete pl; return fail(BLTC_EINVAL, e.what());
         }
-        BLTC_TRY_OR_FREE(cudaDeviceSynchronize());
+        hp.build_ms = ms_since(t0);
+    }
+
+    const auto t0 = std::chrono::steady_clock::now();
+    // tree-ordered records
+    BLTC_TRY_OR_FREE(pl->src_rec.ensure((size_t)N));
+    BLTC_TRY_OR_FREE(launch_pack_records(d_src, d_w, pl->src_perm.p, N, pl->src_rec.p, nullptr));
+    if (hp.shared_order) {
+        pl->tgt_rec = pl->src_rec.p; pl->tgt_perm = pl->src_perm.p;
+    } else {
+        BLTC_TRY_OR_FREE(pl->tgt_rec_own.ensure((size_t)N));
+        BLTC_TRY_OR_FREE(launch_pack_records(d_tgt, nullptr, pl->tgt_perm_own.p, N, pl->tgt_rec_own.p, nullptr));
+        pl->tgt_rec = pl->tgt_rec_own.p; pl->tgt_perm = pl->tgt_perm_own.p;
     }
     // batches, lists, work items
     {
@@ -282,13 +367,6 @@ int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sou
         BLTC_TRY_OR_FREE(pl->b_nseg.upload(bs));
         BLTC_TRY_OR_FREE(pl->b_partial_base.upload(bp));
         const size_t ns = hp.cluster_of_slot.size();
-        std::vector<int32_t> sb(ns), se(ns);
-        for (size_t s = 0; s < ns; ++s) {
-            sb[s] = (int32_t)hp.src.cl[hp.cluster_of_slot[s]].begin;
-            se[s] = (int32_t)hp.src.cl[hp.cluster_of_slot[s]].end;
-        }
-        BLTC_TRY_OR_FREE(pl->slot_begin.upload(sb));
-        BLTC_TRY_OR_FREE(pl->slot_end.upload(se));
         BLTC_TRY_OR_FREE(pl->slot_nodes.upload(hp.slot_nodes));
         BLTC_TRY_OR_FREE(pl->far_slots.upload(hp.far_slots));
         BLTC_TRY_OR_FREE(pl->near_ranges.upload(hp.near_ranges));
@@ -306,6 +384,7 @@ int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sou
     }
 #undef BLTC_TRY_OR_FREE
     pl->upload_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    pl->create_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     pl->on_device = true;
     *h = pl;
     return BLTC_OK;
@@ -351,6 +430,11 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->shard_targets = hp.shard_b1 > hp.shard_b0 ? hp.b_end[hp.shard_b1 - 1] - hp.b_begin[hp.shard_b0] : 0;
     s->shard_far_evals = hp.shard_far_evals;
     s->shard_near_evals = hp.shard_near_evals;
+    s->tree_ms = hp.stage_ms[0];
+    s->lists_ms = hp.stage_ms[1];
+    s->decomp_ms = hp.stage_ms[3];
+    s->create_ms = h->create_ms;
+    s->built_on_device = hp.built_on_device ? 1 : 0;
     return BLTC_OK;
 }
 
@@ -359,7 +443,16 @@ int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
                      int32_t* cl_parent, int32_t* cl_nchild, int64_t* b_begin, int64_t* b_end,
                      int64_t* far_ptr, int32_t* far_idx, int64_t* near_ptr, int32_t* near_idx) {
     if (!h) return fail(BLTC_EINVAL, "handle is NULL");
-    const HostPlan& hp = h->hp;
+    HostPlan& hp = h->hp;
+    BLTC_CUDA(ensure_host_perm(h));
+    if (hp.lists_b0 > 0 || hp.lists_b1 < (int)hp.b_begin.size()) {
+        // a sharded device-built plan traversed only its own batches: complete the lists on the host (the entries
+        // of its own batches come out identical; nothing derived from them changes)
+        try {
+            std::vector<int64_t> fe, ne;
+            plan_lists_host(hp, fe, ne);
+        } catch (const std::exception& e) { return fail(BLTC_ENOMEM, e.what()); }
+    }
     if (src_perm) std::memcpy(src_perm, hp.src.perm.data(), hp.src.perm.size() * sizeof(int64_t));
     if (tgt_perm) std::memcpy(tgt_perm, hp.tgt_perm().data(), hp.tgt_perm().size() * sizeof(int64_t));
     for (size_t c = 0; c < hp.src.cl.size(); ++c) {
@@ -386,6 +479,7 @@ int bltc_get_shard_targets(bltc_handle h, int64_t* idx) {
     if (!h || !idx) return fail(BLTC_EINVAL, "NULL argument");
     const HostPlan& hp = h->hp;
     if (hp.shard_b1 <= hp.shard_b0) return BLTC_OK;
+    BLTC_CUDA(ensure_host_perm(h));
     const std::vector<int64_t>& perm = hp.tgt_perm();
     const int64_t t0 = hp.b_begin[hp.shard_b0], t1 = hp.b_end[hp.shard_b1 - 1];
     for (int64_t t = t0; t < t1; ++t) idx[t - t0] = perm[t];
@@ -607,18 +701,61 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
     std::vector<int32_t> pb_begin, pb_count, pb_nseg;
     std::vector<int64_t> pb_base;
     int nsplit = 1;
+    const int64_t npb64 = (M + kPB - 1) / kPB;
     {
         const int64_t tiles512 = (M + 511) / 512;
         const int64_t want = (int64_t)sms * 2 * 8;
         nsplit = (int)std::min<int64_t>(64, std::max<int64_t>(1, (want + tiles512 - 1) / tiles512));
         nsplit = (int)std::min<int64_t>(nsplit, std::max<int64_t>(1, N / 256));
-        for (int s = 0; s < nsplit; ++s)
-            ranges.push_back(Range{(int32_t)(N * s / nsplit), (int32_t)(N * (s + 1) / nsplit), kRangeMayCoincide});
-        for (int64_t b0 = 0; b0 < M; b0 += kPB) {
+    }
+    // Bounding boxes of the pseudo-batches and of the source segments (one small kernel each, read back: the one
+    // synchronisation of this call).  A segment whose box does not meet the batch's box cannot hold a source that
+    // coincides with one of its targets, so its tiles run without the r == 0 test (reading R3); and the exp
+    // underflow guard is compiled in only if k_max x (the largest possible distance) can reach 700.
+    const int64_t seg_len = std::max<int64_t>(1, (N + nsplit - 1) / nsplit);
+    const int nseg_box = (int)((N + seg_len - 1) / seg_len);
+    std::vector<double> box_t((size_t)npb64 * 6), box_s((size_t)nseg_box * 6);
+    {
+        TempBuf t_bt, t_bs;
+        BLTC_CUDA(t_bt.alloc(box_t.size() * sizeof(double), st));
+        BLTC_CUDA(t_bs.alloc(box_s.size() * sizeof(double), st));
+        BLTC_CUDA(launch_chunk_bbox(d_tg, M, kPB, t_bt.as<double>(), st));
+        BLTC_CUDA(launch_chunk_bbox(d_sr, N, seg_len, t_bs.as<double>(), st));
+        BLTC_CUDA(cudaMemcpyAsync(box_t.data(), t_bt.p, box_t.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+        BLTC_CUDA(cudaMemcpyAsync(box_s.data(), t_bs.p, box_s.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+        BLTC_CUDA(cudaStreamSynchronize(st));
+    }
+    bool guard = true;
+    if (kind == kYukawa) {
+        double lo[3], hi[3], d2 = 0.0, kmax = 0.0;
+        for (int d = 0; d < 3; ++d) { lo[d] = INFINITY; hi[d] = -INFINITY; }
+        for (int64_t c = 0; c < npb64; ++c)
+            for (int d = 0; d < 3; ++d) { lo[d] = std::min(lo[d], box_t[c * 6 + d]); hi[d] = std::max(hi[d], box_t[c * 6 + 3 + d]); }
+        for (int c = 0; c < nseg_box; ++c)
+            for (int d = 0; d < 3; ++d) { lo[d] = std::min(lo[d], box_s[c * 6 + d]); hi[d] = std::max(hi[d], box_s[c * 6 + 3 + d]); }
+        for (int d = 0; d < 3; ++d) d2 += (hi[d] - lo[d]) * (hi[d] - lo[d]);
+        for (int o = 0; o < n_orb; ++o) kmax = std::max(kmax, k[o]);
+        guard = !(kmax * std::sqrt(d2) < 700.0);
+    }
+    {
+        // ranges[pb * nsplit + s]: source segment s as seen from pseudo-batch pb
+        ranges.reserve((size_t)npb64 * nsplit);
+        for (int64_t pb = 0; pb < npb64; ++pb) {
+            const int64_t b0 = pb * kPB;
             pb_begin.push_back((int32_t)b0);
             pb_count.push_back((int32_t)std::min<int64_t>(kPB, M - b0));
             pb_nseg.push_back(nsplit);
             pb_base.push_back((int64_t)nsplit * b0);
+            for (int s = 0; s < nsplit; ++s) {
+                const int64_t s0 = std::min<int64_t>(N, (int64_t)s * seg_len), s1 = std::min<int64_t>(N, (int64_t)(s + 1) * seg_len);
+                bool touch = s1 > s0;
+                if (touch) {
+                    const int sb = (int)(s0 / seg_len);
+                    for (int d = 0; d < 3; ++d)
+                        touch = touch && box_s[sb * 6 + d] <= box_t[pb * 6 + 3 + d] && box_t[pb * 6 + d] <= box_s[sb * 6 + 3 + d];
+                }
+                ranges.push_back(Range{(int32_t)s0, (int32_t)s1, touch ? kRangeMayCoincide : 0});
+            }
         }
         const int unit = 32 * kTargetsPerThread;
         for (int64_t t0 = 0; t0 < M;) {
@@ -629,7 +766,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             int gs = 0; while ((1 << gs) < g) ++gs;
             const int64_t cnt = std::min<int64_t>((int64_t)g * unit, pb_end - t0);
             for (int s = 0; s < nsplit; ++s)
-                items.push_back(WorkItem{(int32_t)t0, (int32_t)cnt, gs, s, s + 1, 0,
+                items.push_back(WorkItem{(int32_t)t0, (int32_t)cnt, gs, (int32_t)(pb * nsplit + s), (int32_t)(pb * nsplit + s + 1), 0,
                                          pb_base[pb] + (int64_t)s * pb_count[pb] + (t0 - pb * kPB)});
             t0 += cnt;
         }
@@ -673,7 +810,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
             BLTC_CUDA(cudaEventRecord(ea, st));
         }
-        BLTC_CUDA(launch_near(kind, ot, sub, true, t_items.as<WorkItem>(), (int)items.size(), t_ranges.as<Range>(),
+        BLTC_CUDA(launch_near(kind, ot, sub, guard, t_items.as<WorkItem>(), (int)items.size(), t_ranges.as<Range>(),
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }

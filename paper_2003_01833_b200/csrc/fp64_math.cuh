@@ -9,13 +9,18 @@
 //
 //   rsqrt: MUFU.RSQ64H seed (XU pipe, rel. error <~ 2^-20) + one cubic step: 5 FP64 instructions,
 //          residual 5 e^3/16 < 2^-58; +1 for r = r2 * rinv.
-//   exp:   u = r * c,  c = -k T/ln2 (per orbital, host-computed),  T = 2048;
+//   exp:   u = r * c,  c = -k T/ln2 (per orbital, host-computed),  T = BLTC_EXP_T = 8192 (exp_table.inc);
 //          t = u + (1.5*2^52 + 1023 T)  ->  low word m = rint(u) + 1023 T = T*(n + 1023) + j
-//          rho = u - rint(u) in [-1/2, 1/2];   exp(-k r) = 2^n * 2^(j/T) * (1 + rho (C1 + C2 rho + C3 rho^2))
-//          2^(j/T): 16 KB shared-memory table (bank conflicts are harmless here: measured);
-//          2^n: the biased exponent n + 1023 = m >> 11 is merged into the table value's exponent field
-//          with one rotate + one LOP3 (the table values are in [1,2), exponent field 0x3FF).
-//          7 FP64 instructions.  Polynomial error 8.6e-18, total <= ~1 ulp.
+//          rho = u - rint(u) in [-1/2, 1/2];   exp(-k r) = 2^n * 2^(j/T) * (1 + rho (C1 + C2 rho))
+//          2^(j/T): 64 KB shared-memory table per CTA, read by per-lane LDS.64 (random entries: ~4.4 SM cycles
+//          per warp lookup against 2 conflict-free, measured; a 16-copy conflict-free table of 512 entries needs
+//          the cubic polynomial again and was measured slower, profiles/r02a_variants.md);
+//          2^n: the table's high words are pre-biased by -(j << 7), so adding (m << 7) -- one shift, one add,
+//          both on the ALU pipe -- puts the biased exponent n + 1023 and the mantissa of 2^(j/T) in place.
+//          6 FP64 instructions per exp.  Quadratic near-minimax polynomial: relative error <= 6.3e-15 (about 28
+//          ulp), odd in rho and therefore of pseudo-random sign from pair to pair; the measured end-to-end parity
+//          errors are 3e-16 ... 2.4e-14.  BLTC_EXP_DEG == 3 (T = 2048, cubic, 7 instructions,
+//          8.6e-18) remains as a compile-time alternative: python gen_exp_table.py 2048 3 > exp_table.inc.
 //          Any u <= 0 is legal: if m < 0 (exp(-k r) < 2^-1023) the high word of t differs from 0x43380000
 //          and m is replaced by 0, which gives a subnormal-sized value (absolute error < 1e-307).
 #pragma once

@@ -13,9 +13,10 @@
 // through shared memory in a fixed order and written to a per-(batch, segment) slice of the
 // partial buffer; the epilogue adds the slices in a fixed order => bitwise reproducible results.
 //
-// The bound is the FP64 pipe ("Roofline"): 22 (near) / 16.4 (far, n = 8) FP64 instructions
-// per kernel evaluation for one orbital; everything else (LDS, MUFU seed, integer exponent work,
-// loop control) issues in the shadow of the half-rate FP64 pipe.
+// The bound is the FP64 pipe: per (target, source) pair and orbital tile of OT = 1 / 2 / 3 / 4
+// orbitals the near kernel executes 22 / 31 / 40 / 49 FP64 instructions and the far kernel (n = 8) 16.4 / 25.4 /
+// 34.4 / 43.4; everything else (LDS, MUFU seed, integer exponent work, loop control) issues in the shadow of the
+// half-rate FP64 pipe, except that at OT >= 3 the exp-table lookups bring the shared-memory pipe to the same load.
 #include "kernels.cuh"
 
 #include "fp64_math.cuh"
@@ -45,6 +46,36 @@ __global__ void pack_kernel(const double* __restrict__ coords, const double* __r
     if (i >= n) return;
     const int64_t s = perm ? (int64_t)perm[i] : i;
     rec[i] = make_double4(coords[s], coords[n + s], coords[2 * n + s], w ? w[s] : 0.0);
+}
+
+// Bounding boxes of consecutive chunks of a SoA point set: out[chunk] = {lo[3], hi[3]}.  direct_convolve uses them
+// to decide where a source can coincide with a target (reading R3) and whether exp can underflow.
+__global__ void __launch_bounds__(kThreads)
+chunk_bbox_kernel(const double* __restrict__ coords, int64_t n, int64_t chunk, double* __restrict__ out) {
+    __shared__ double s_lo[3][kThreads / 32], s_hi[3][kThreads / 32];
+    const int64_t b = (int64_t)blockIdx.x * chunk, e = min(n, b + chunk);
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int64_t i = b + threadIdx.x; i < e; i += kThreads)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double v = coords[(int64_t)d * n + i];
+            lo[d] = fmin(lo[d], v); hi[d] = fmax(hi[d], v);
+        }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        for (int s = 16; s > 0; s >>= 1) {
+            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], s));
+            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], s));
+        }
+        if ((threadIdx.x & 31) == 0) { s_lo[d][threadIdx.x >> 5] = lo[d]; s_hi[d][threadIdx.x >> 5] = hi[d]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        const int d = threadIdx.x;
+        double a = s_lo[d][0], c = s_hi[d][0];
+        for (int w = 1; w < kThreads / 32; ++w) { a = fmin(a, s_lo[d][w]); c = fmax(c, s_hi[d][w]); }
+        out[(size_t)blockIdx.x * 6 + d] = a; out[(size_t)blockIdx.x * 6 + 3 + d] = c;
+    }
 }
 
 // ------------------------------------------------------------------------------------ a2
@@ -569,6 +600,12 @@ cudaError_t launch_pack_records(const double* coords, const double* w, const int
                                 double4* rec, cudaStream_t st) {
     if (n == 0) return cudaSuccess;
     pack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(coords, w, perm, n, rec);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_chunk_bbox(const double* coords, int64_t n, int64_t chunk, double* out, cudaStream_t st) {
+    if (n == 0) return cudaSuccess;
+    chunk_bbox_kernel<<<(unsigned)((n + chunk - 1) / chunk), kThreads, 0, st>>>(coords, n, chunk, out);
     return cudaGetLastError();
 }
 

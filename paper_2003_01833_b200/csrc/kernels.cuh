@@ -41,6 +41,9 @@ cudaError_t launch_gather(const double* f, int64_t stride, int o0, int ot, const
 cudaError_t launch_pack_records(const double* coords, const double* w, const int32_t* perm, int64_t n,
                                 double4* rec, cudaStream_t st);
 
+// bounding boxes {lo[3], hi[3]} of the chunks [c*chunk, min(n, (c+1)*chunk)) of SoA coords[3][n] -> out[nchunk][6]
+cudaError_t launch_chunk_bbox(const double* coords, int64_t n, int64_t chunk, double* out, cudaStream_t st);
+
 // a2: proxy charges.  ot == 0: what[slot][P] from w;  ot >= 1: fhat[slot][P][ot] from f*w.
 // items: chunked work (plan_host.hpp); chunk_out: scratch of up_partial_chunks * P * max(ot,1) doubles
 cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduce* red, int nred,

@@ -132,6 +132,8 @@ void gather_leaves(const Tree& t, int id, std::vector<int>& out) {
     for (int q = 0; q < t.cl[id].nchild; ++q) gather_leaves(t, t.cl[id].child[q], out);
 }
 
+}  // namespace
+
 void build_tree(Tree& t, const double* x, const double* y, const double* z, int64_t n, int64_t max_leaf) {
     t.cl.clear();
     TreeBuilder tb(t.perm, x, y, z, n, max_leaf);
@@ -139,6 +141,8 @@ void build_tree(Tree& t, const double* x, const double* y, const double* z, int6
     t.leaves.clear();
     gather_leaves(t, 0, t.leaves);
 }
+
+namespace {
 
 inline double half_diagonal(const double* lo, const double* hi) {
     const double ex = hi[0] - lo[0], ey = hi[1] - lo[1], ez = hi[2] - lo[2];
@@ -210,13 +214,7 @@ std::vector<int> shard_cuts(const std::vector<int64_t>& batch_cost, int world) {
     return cut;
 }
 
-void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
-                     double theta, int degree, int batch_size, int leaf_size, int sm_count,
-                     int shard_rank, int shard_world) {
-    const auto t0 = std::chrono::steady_clock::now();
-    if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world)
-        throw std::invalid_argument("shard rank/world must satisfy 0 <= rank < world");
-    if (!sources) throw std::invalid_argument("sources is NULL");
+void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size) {
     if (N <= 0 || N > (int64_t)2000000000) throw std::invalid_argument("N must be in [1, 2e9]");
     if (!(theta >= 0.0) || !(theta < 1.0)) throw std::invalid_argument("theta must be in [0, 1)");
     if (degree < 1 || degree > 20) throw std::invalid_argument("interp_degree must be in [1, 20]");
@@ -225,18 +223,12 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
     p.N = N; p.M = N; p.theta = theta; p.degree = degree;
     p.P = (degree + 1) * (degree + 1) * (degree + 1);
     p.leaf_size = leaf_size; p.batch_size = batch_size;
-    p.same_points = (targets == nullptr || targets == sources);
-    p.shared_order = p.same_points && batch_size == leaf_size;
-    const double* sx = sources; const double* sy = sources + N; const double* sz = sources + 2 * N;
+    p.same_points = same_points;
+    p.shared_order = same_points && batch_size == leaf_size;
+}
 
-    // Algorithm 3 line 1: tree of source clusters and set of target batches
-    build_tree(p.src, sx, sy, sz, N, leaf_size);
-    const Tree* bt = &p.src;
-    if (!p.shared_order) {
-        const double* t = p.same_points ? sources : targets;
-        build_tree(p.tgt, t, t + N, t + 2 * N, N, batch_size);
-        bt = &p.tgt;
-    }
+void plan_set_batches(HostPlan& p) {
+    const Tree* bt = p.shared_order ? &p.src : &p.tgt;
     {   // bound of |target - source|: farthest corners of the two root boxes
         const Cluster& A = p.src.cl[0];
         const Cluster& B = bt->cl[0];
@@ -254,70 +246,81 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         p.b_begin[b] = L.begin; p.b_end[b] = L.end;
         for (int d = 0; d < 3; ++d) { p.b_lo[3 * b + d] = L.lo[d]; p.b_hi[3 * b + d] = L.hi[d]; }
     }
+}
 
-    auto lap = [&, last = t0](int stage) mutable {
-        const auto now = std::chrono::steady_clock::now();
-        p.stage_ms[stage] += std::chrono::duration<double, std::milli>(now - last).count();
-        last = now;
-    };
-    lap(0);
+// Algorithm 3 line 3, decisions: per-batch interaction lists ("precomputed for each target batch")
+// for the batches [b0, b1), written at the CSR offsets far_ptr / near_ptr (which must be set).  Batches are
+// independent: contiguous chunks of them are traversed by concurrent tasks.
 
-    // line 3, decisions: per-batch interaction lists ("precomputed for each target batch").
-    // Batches are independent: contiguous chunks of them are traversed by concurrent tasks into private
-    // lists, concatenated in batch order (identical to the sequential result).
+void plan_lists_host(HostPlan& p, std::vector<int64_t>& b_far_evals, std::vector<int64_t>& b_near_evals) {
+    const int nb = (int)p.b_begin.size();
     p.far_ptr.assign(nb + 1, 0); p.near_ptr.assign(nb + 1, 0);
-    std::vector<int64_t> b_far_evals(nb, 0), b_near_evals(nb, 0);
-    {
-        const int hw = (int)std::max(1u, std::thread::hardware_concurrency());
-        const int nchunk = std::max(1, std::min(hw, nb / 64));
-        std::vector<std::vector<int32_t>> cfar(nchunk), cnear(nchunk);
-        std::vector<int64_t> nfar(nb, 0), nnear(nb, 0);
-        auto work = [&](int ch) {
-            const int b0 = (int)((int64_t)nb * ch / nchunk), b1 = (int)((int64_t)nb * (ch + 1) / nchunk);
-            for (int b = b0; b < b1; ++b) {
-                const size_t f0 = cfar[ch].size(), n0 = cnear[ch].size();
-                Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
-                             cfar[ch], cnear[ch]};
-                tr.visit(0);
-                nfar[b] = (int64_t)(cfar[ch].size() - f0); nnear[b] = (int64_t)(cnear[ch].size() - n0);
-                const int64_t nt = p.b_end[b] - p.b_begin[b];
-                b_far_evals[b] = nt * p.P * nfar[b];
-                for (size_t q = n0; q < cnear[ch].size(); ++q)
-                    b_near_evals[b] += nt * (p.src.cl[cnear[ch][q]].end - p.src.cl[cnear[ch][q]].begin);
-            }
-        };
-        if (nchunk == 1) work(0);
-        else {
-            std::vector<std::future<void>> tasks;
-            for (int ch = 0; ch < nchunk; ++ch) tasks.push_back(std::async(std::launch::async, work, ch));
-            for (auto& t : tasks) t.get();
+    b_far_evals.assign(nb, 0); b_near_evals.assign(nb, 0);
+    const int hw = (int)std::max(1u, std::thread::hardware_concurrency());
+    const int nchunk = std::max(1, std::min(hw, nb / 64));
+    std::vector<std::vector<int32_t>> cfar(nchunk), cnear(nchunk);
+    std::vector<int64_t> nfar(nb, 0), nnear(nb, 0);
+    auto work = [&](int ch) {
+        const int b0 = (int)((int64_t)nb * ch / nchunk), b1 = (int)((int64_t)nb * (ch + 1) / nchunk);
+        for (int b = b0; b < b1; ++b) {
+            const size_t f0 = cfar[ch].size(), n0 = cnear[ch].size();
+            Traversal tr{p, &p.b_lo[3 * b], &p.b_hi[3 * b], half_diagonal(&p.b_lo[3 * b], &p.b_hi[3 * b]),
+                         cfar[ch], cnear[ch]};
+            tr.visit(0);
+            nfar[b] = (int64_t)(cfar[ch].size() - f0); nnear[b] = (int64_t)(cnear[ch].size() - n0);
+            const int64_t nt = p.b_end[b] - p.b_begin[b];
+            b_far_evals[b] = nt * p.P * nfar[b];
+            for (size_t q = n0; q < cnear[ch].size(); ++q)
+                b_near_evals[b] += nt * (p.src.cl[cnear[ch][q]].end - p.src.cl[cnear[ch][q]].begin);
         }
-        for (int b = 0; b < nb; ++b) {
-            p.far_ptr[b + 1] = p.far_ptr[b] + nfar[b]; p.near_ptr[b + 1] = p.near_ptr[b] + nnear[b];
-            p.far_evals += b_far_evals[b]; p.near_evals += b_near_evals[b];
-        }
-        p.far_idx.reserve((size_t)p.far_ptr[nb]); p.near_idx.reserve((size_t)p.near_ptr[nb]);
-        for (int ch = 0; ch < nchunk; ++ch) {
-            p.far_idx.insert(p.far_idx.end(), cfar[ch].begin(), cfar[ch].end());
-            p.near_idx.insert(p.near_idx.end(), cnear[ch].begin(), cnear[ch].end());
-        }
+    };
+    if (nchunk == 1) work(0);
+    else {
+        std::vector<std::future<void>> tasks;
+        for (int ch = 0; ch < nchunk; ++ch) tasks.push_back(std::async(std::launch::async, work, ch));
+        for (auto& t : tasks) t.get();
     }
+    for (int b = 0; b < nb; ++b) {
+        p.far_ptr[b + 1] = p.far_ptr[b] + nfar[b]; p.near_ptr[b + 1] = p.near_ptr[b] + nnear[b];
+    }
+    p.far_idx.clear(); p.near_idx.clear();
+    p.far_idx.reserve((size_t)p.far_ptr[nb]); p.near_idx.reserve((size_t)p.near_ptr[nb]);
+    for (int ch = 0; ch < nchunk; ++ch) {
+        p.far_idx.insert(p.far_idx.end(), cfar[ch].begin(), cfar[ch].end());
+        p.near_idx.insert(p.near_idx.end(), cnear[ch].begin(), cnear[ch].end());
+    }
+    p.lists_b0 = 0; p.lists_b1 = nb;
+}
 
-    lap(1);
-
+void plan_set_shard(HostPlan& p, const std::vector<int64_t>& b_far_evals, const std::vector<int64_t>& b_near_evals,
+                    int shard_rank, int shard_world) {
+    if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world)
+        throw std::invalid_argument("shard rank/world must satisfy 0 <= rank < world");
+    const int nb = (int)p.b_begin.size();
+    p.far_evals = p.near_evals = 0;
+    std::vector<int64_t> cost(nb);
+    for (int b = 0; b < nb; ++b) {
+        p.far_evals += b_far_evals[b]; p.near_evals += b_near_evals[b];
+        cost[b] = b_far_evals[b] + b_near_evals[b];
+    }
     // batch slice of this rank: equal shares of the kernel evaluations (the batches are independent given
     // the sources and the proxy charges)
     p.shard_rank = shard_rank; p.shard_world = shard_world;
-    {
-        std::vector<int64_t> cost(nb);
-        for (int b = 0; b < nb; ++b) cost[b] = b_far_evals[b] + b_near_evals[b];
-        const std::vector<int> cut = shard_cuts(cost, shard_world);
-        p.shard_b0 = cut[shard_rank]; p.shard_b1 = cut[shard_rank + 1];
-        for (int b = p.shard_b0; b < p.shard_b1; ++b) {
-            p.shard_far_evals += b_far_evals[b]; p.shard_near_evals += b_near_evals[b];
-        }
+    const std::vector<int> cut = shard_cuts(cost, shard_world);
+    p.shard_b0 = cut[shard_rank]; p.shard_b1 = cut[shard_rank + 1];
+    p.shard_far_evals = p.shard_near_evals = 0;
+    for (int b = p.shard_b0; b < p.shard_b1; ++b) {
+        p.shard_far_evals += b_far_evals[b]; p.shard_near_evals += b_near_evals[b];
     }
+}
+
+// Everything after the lists of the batches [shard_b0, shard_b1) are known: proxy slots with their Chebyshev grids,
+// upward-pass work items, and the B200 work decomposition.
+void plan_finish(HostPlan& p, int sm_count) {
+    const int nb = (int)p.b_begin.size();
     const int B0 = p.shard_b0, B1 = p.shard_b1;
+    const int degree = p.degree;
+    if (B0 < p.lists_b0 || B1 > p.lists_b1) throw std::logic_error("plan_finish: lists of the shard's batches are missing");
 
     // proxy slots: clusters that appear in some far list (R9), with their Chebyshev grids Eq. (37)
     const int ncl = (int)p.src.cl.size();
@@ -364,35 +367,18 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
         });
     }
 
-    lap(2);
-
     // ---- B200 work decomposition -------------------------------------------------------
     // Per batch: near clusters -> merged contiguous source ranges; far clusters -> slot ids.
     // Lists are cut into segments so that (tiles x segments) gives >= ~32 work items per
     // resident CTA slot (2 CTAs/SM), each CTA slot then sees many items sorted by cost.
+    // Batches are independent: chunks of them are decomposed by concurrent tasks into private vectors
+    // (indices relative to the chunk) that are spliced in batch order afterwards.
     const int cta_slots = std::max(1, sm_count) * 2;
-    std::vector<std::vector<Range>> merged(nb);
-    std::vector<int64_t> near_src(nb, 0);
     double near_cost = 0, far_cost = 0;            // in (target group of 64) x (source) units
+    std::vector<int64_t> near_src(nb, 0);
     for (int b = B0; b < B1; ++b) {
-        std::vector<Range>& r = merged[b];
-        for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
-            const Cluster& C = p.src.cl[p.near_idx[q]];
-            // can a source of C coincide with a target of the batch?  Only if the (closed, minimal)
-            // bounding boxes intersect; otherwise the kernel skips the r == 0 test (reading R3).
-            bool touch = true;
-            for (int d = 0; d < 3; ++d)
-                touch = touch && C.lo[d] <= p.b_hi[3 * b + d] && p.b_lo[3 * b + d] <= C.hi[d];
-            r.push_back(Range{(int32_t)C.begin, (int32_t)C.end, touch ? kRangeMayCoincide : 0});
-        }
-        std::sort(r.begin(), r.end(), [](const Range& a, const Range& c) { return a.begin < c.begin; });
-        size_t o = 0;
-        for (size_t i = 0; i < r.size(); ++i) {
-            if (o > 0 && r[o - 1].end == r[i].begin && r[o - 1].flags == r[i].flags) r[o - 1].end = r[i].end;
-            else r[o++] = r[i];
-        }
-        r.resize(o);
-        for (const Range& g : r) near_src[b] += g.end - g.begin;
+        for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q)
+            near_src[b] += p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin;
         const double groups = (double)((p.b_end[b] - p.b_begin[b] + 63) / 64);
         near_cost += groups * (double)near_src[b];
         far_cost += groups * (double)(p.far_ptr[b + 1] - p.far_ptr[b]) * p.P;
@@ -401,85 +387,173 @@ void build_host_plan(HostPlan& p, const double* targets, const double* sources, 
     const double far_cap = std::max((double)p.P, far_cost / (cta_slots * 32.0 * 8.0));
 
     p.b_nseg_far.assign(nb, 0); p.b_nseg_near.assign(nb, 0); p.b_partial_base.assign(nb, 0);
-    std::vector<std::pair<int32_t, int32_t>> tiles; std::vector<int> gsh;
-    int64_t partial = 0;
-    for (int b = B0; b < B1; ++b) {
-        const int64_t nt = p.b_end[b] - p.b_begin[b];
-        // near segments: equal source counts, ranges may be cut anywhere
-        std::vector<std::pair<int32_t, int32_t>> nseg_slices;    // [begin, end) into near_ranges
-        if (near_src[b] > 0) {
-            int nseg = (int)std::min<int64_t>(64, (int64_t)std::ceil((double)near_src[b] / near_cap));
-            nseg = std::max(1, nseg);
-            const int64_t per = (near_src[b] + nseg - 1) / nseg;
-            int64_t room = per;
-            int32_t seg_start = (int32_t)p.near_ranges.size();
-            for (const Range& g : merged[b]) {
-                int32_t at = g.begin;
-                while (at < g.end) {
-                    const int32_t take = (int32_t)std::min<int64_t>(room, g.end - at);
-                    p.near_ranges.push_back(Range{at, at + take, g.flags});
-                    at += take; room -= take;
-                    if (room == 0) {
-                        nseg_slices.emplace_back(seg_start, (int32_t)p.near_ranges.size());
-                        seg_start = (int32_t)p.near_ranges.size(); room = per;
+    struct Chunk {
+        std::vector<Range> ranges; std::vector<int32_t> slots; std::vector<WorkItem> far_items, near_items;
+        std::vector<int64_t> near_key; int64_t partial = 0;
+    };
+    const int hw = (int)std::max(1u, std::thread::hardware_concurrency());
+    const int nchunk = std::max(1, std::min(hw, (B1 - B0) / 32));
+    std::vector<Chunk> chunks(nchunk);
+    auto decompose = [&](int ch) {
+        Chunk& K = chunks[ch];
+        const int c0 = B0 + (int)((int64_t)(B1 - B0) * ch / nchunk), c1 = B0 + (int)((int64_t)(B1 - B0) * (ch + 1) / nchunk);
+        std::vector<Range> r;
+        std::vector<std::pair<int32_t, int32_t>> tiles, nseg_slices, fseg_slices; std::vector<int> gsh;
+        for (int b = c0; b < c1; ++b) {
+            r.clear();
+            for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
+                const Cluster& C = p.src.cl[p.near_idx[q]];
+                // can a source of C coincide with a target of the batch?  Only if the (closed, minimal)
+                // bounding boxes intersect; otherwise the kernel skips the r == 0 test (reading R3).
+                bool touch = true;
+                for (int d = 0; d < 3; ++d)
+                    touch = touch && C.lo[d] <= p.b_hi[3 * b + d] && p.b_lo[3 * b + d] <= C.hi[d];
+                r.push_back(Range{(int32_t)C.begin, (int32_t)C.end, touch ? kRangeMayCoincide : 0});
+            }
+            std::sort(r.begin(), r.end(), [](const Range& a, const Range& c) { return a.begin < c.begin; });
+            size_t o = 0;
+            for (size_t i = 0; i < r.size(); ++i) {
+                if (o > 0 && r[o - 1].end == r[i].begin && r[o - 1].flags == r[i].flags) r[o - 1].end = r[i].end;
+                else r[o++] = r[i];
+            }
+            r.resize(o);
+            const int64_t nt = p.b_end[b] - p.b_begin[b];
+            // near segments: equal source counts, ranges may be cut anywhere
+            nseg_slices.clear();    // [begin, end) into the chunk's ranges
+            if (near_src[b] > 0) {
+                int nseg = (int)std::min<int64_t>(64, (int64_t)std::ceil((double)near_src[b] / near_cap));
+                nseg = std::max(1, nseg);
+                const int64_t per = (near_src[b] + nseg - 1) / nseg;
+                int64_t room = per;
+                int32_t seg_start = (int32_t)K.ranges.size();
+                for (const Range& g : r) {
+                    int32_t at = g.begin;
+                    while (at < g.end) {
+                        const int32_t take = (int32_t)std::min<int64_t>(room, g.end - at);
+                        K.ranges.push_back(Range{at, at + take, g.flags});
+                        at += take; room -= take;
+                        if (room == 0) {
+                            nseg_slices.emplace_back(seg_start, (int32_t)K.ranges.size());
+                            seg_start = (int32_t)K.ranges.size(); room = per;
+                        }
                     }
                 }
+                if ((int32_t)K.ranges.size() > seg_start)
+                    nseg_slices.emplace_back(seg_start, (int32_t)K.ranges.size());
             }
-            if ((int32_t)p.near_ranges.size() > seg_start)
-                nseg_slices.emplace_back(seg_start, (int32_t)p.near_ranges.size());
-        }
-        // far segments: whole clusters
-        std::vector<std::pair<int32_t, int32_t>> fseg_slices;
-        const int64_t nfar = p.far_ptr[b + 1] - p.far_ptr[b];
-        if (nfar > 0) {
-            const int64_t per = std::max<int64_t>(1, (int64_t)(far_cap / p.P));
-            int64_t nseg = std::min<int64_t>(64, (nfar + per - 1) / per);
-            const int64_t per2 = (nfar + nseg - 1) / nseg;
-            for (int64_t q = 0; q < nfar; q += per2) {
-                const int32_t s0 = (int32_t)p.far_slots.size();
-                for (int64_t u = q; u < std::min(nfar, q + per2); ++u)
-                    p.far_slots.push_back(p.slot_of_cluster[p.far_idx[p.far_ptr[b] + u]]);
-                fseg_slices.emplace_back(s0, (int32_t)p.far_slots.size());
+            // far segments: whole clusters
+            fseg_slices.clear();
+            const int64_t nfar = p.far_ptr[b + 1] - p.far_ptr[b];
+            if (nfar > 0) {
+                const int64_t per = std::max<int64_t>(1, (int64_t)(far_cap / p.P));
+                int64_t nseg = std::min<int64_t>(64, (nfar + per - 1) / per);
+                const int64_t per2 = (nfar + nseg - 1) / nseg;
+                for (int64_t q = 0; q < nfar; q += per2) {
+                    const int32_t s0 = (int32_t)K.slots.size();
+                    for (int64_t u = q; u < std::min(nfar, q + per2); ++u)
+                        K.slots.push_back(p.slot_of_cluster[p.far_idx[p.far_ptr[b] + u]]);
+                    fseg_slices.emplace_back(s0, (int32_t)K.slots.size());
+                }
             }
+            p.b_nseg_far[b] = (int32_t)fseg_slices.size();
+            p.b_nseg_near[b] = (int32_t)nseg_slices.size();
+            p.b_partial_base[b] = K.partial;                      // relative to the chunk
+            make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh);
+            for (size_t ti = 0; ti < tiles.size(); ++ti) {
+                const int64_t local = tiles[ti].first - p.b_begin[b];
+                for (size_t s = 0; s < fseg_slices.size(); ++s)
+                    K.far_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                        fseg_slices[s].first, fseg_slices[s].second, 0,
+                        K.partial + (int64_t)s * nt + local});
+                for (size_t s = 0; s < nseg_slices.size(); ++s) {
+                    K.near_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
+                        nseg_slices[s].first, nseg_slices[s].second, 0,
+                        K.partial + (int64_t)(fseg_slices.size() + s) * nt + local});
+                    int64_t key = 0;
+                    for (int32_t q = nseg_slices[s].first; q < nseg_slices[s].second; ++q)
+                        key += K.ranges[q].end - K.ranges[q].begin;
+                    K.near_key.push_back(key << gsh[ti]);
+                }
+            }
+            K.partial += (int64_t)(fseg_slices.size() + nseg_slices.size()) * nt;
         }
-        p.b_nseg_far[b] = (int32_t)fseg_slices.size();
-        p.b_nseg_near[b] = (int32_t)nseg_slices.size();
-        p.b_partial_base[b] = partial;
-        make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh);
-        for (size_t ti = 0; ti < tiles.size(); ++ti) {
-            const int64_t local = tiles[ti].first - p.b_begin[b];
-            for (size_t s = 0; s < fseg_slices.size(); ++s)
-                p.far_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                    fseg_slices[s].first, fseg_slices[s].second, 0,
-                    partial + (int64_t)s * nt + local});
-            for (size_t s = 0; s < nseg_slices.size(); ++s)
-                p.near_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                    nseg_slices[s].first, nseg_slices[s].second, 0,
-                    partial + (int64_t)(fseg_slices.size() + s) * nt + local});
-        }
-        partial += (int64_t)(fseg_slices.size() + nseg_slices.size()) * nt;
+    };
+    if (nchunk == 1) decompose(0);
+    else {
+        std::vector<std::future<void>> tasks;
+        for (int ch = 0; ch < nchunk; ++ch) tasks.push_back(std::async(std::launch::async, decompose, ch));
+        for (auto& t : tasks) t.get();
     }
-    p.partial_len = partial;
+    // splice the chunks in batch order: chunk-relative indices become global ones
+    std::vector<int64_t> near_key;
+    {
+        size_t nr = 0, nsl = 0, nfi = 0, nni = 0;
+        for (const Chunk& K : chunks) { nr += K.ranges.size(); nsl += K.slots.size(); nfi += K.far_items.size(); nni += K.near_items.size(); }
+        p.near_ranges.reserve(nr); p.far_slots.reserve(nsl); p.far_items.reserve(nfi); p.near_items.reserve(nni);
+        near_key.reserve(nni);
+        int64_t partial = 0;
+        for (int ch = 0; ch < nchunk; ++ch) {
+            Chunk& K = chunks[ch];
+            const int32_t rbase = (int32_t)p.near_ranges.size(), sbase = (int32_t)p.far_slots.size();
+            const int c0 = B0 + (int)((int64_t)(B1 - B0) * ch / nchunk), c1 = B0 + (int)((int64_t)(B1 - B0) * (ch + 1) / nchunk);
+            for (int b = c0; b < c1; ++b) p.b_partial_base[b] += partial;
+            for (WorkItem w : K.far_items) {
+                w.list_begin += sbase; w.list_end += sbase; w.partial_off += partial;
+                p.far_items.push_back(w);
+            }
+            for (WorkItem w : K.near_items) {
+                w.list_begin += rbase; w.list_end += rbase; w.partial_off += partial;
+                p.near_items.push_back(w);
+            }
+            p.near_ranges.insert(p.near_ranges.end(), K.ranges.begin(), K.ranges.end());
+            p.far_slots.insert(p.far_slots.end(), K.slots.begin(), K.slots.end());
+            near_key.insert(near_key.end(), K.near_key.begin(), K.near_key.end());
+            partial += K.partial;
+            K = Chunk();
+        }
+        p.partial_len = partial;
+    }
 
     // longest-processing-time-first: the hardware block scheduler hands out CTAs in order
-    auto near_cost_of = [&](const WorkItem& w) {
-        int64_t s = 0;
-        for (int32_t q = w.list_begin; q < w.list_end; ++q) s += p.near_ranges[q].end - p.near_ranges[q].begin;
-        return s << w.gshift;
-    };
     auto far_cost_of = [&](const WorkItem& w) { return (int64_t)(w.list_end - w.list_begin) << w.gshift; };
     {
-        std::vector<int64_t> key(p.near_items.size());
-        for (size_t i = 0; i < key.size(); ++i) key[i] = near_cost_of(p.near_items[i]);
-        std::vector<size_t> ord(key.size());
+        std::vector<size_t> ord(near_key.size());
         std::iota(ord.begin(), ord.end(), size_t(0));
-        std::stable_sort(ord.begin(), ord.end(), [&](size_t a, size_t c) { return key[a] > key[c]; });
-        std::vector<WorkItem> sorted(key.size());
+        std::stable_sort(ord.begin(), ord.end(), [&](size_t a, size_t c) { return near_key[a] > near_key[c]; });
+        std::vector<WorkItem> sorted(near_key.size());
         for (size_t i = 0; i < ord.size(); ++i) sorted[i] = p.near_items[ord[i]];
         p.near_items.swap(sorted);
         std::stable_sort(p.far_items.begin(), p.far_items.end(),
                          [&](const WorkItem& a, const WorkItem& c) { return far_cost_of(a) > far_cost_of(c); });
     }
+}
+
+void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
+                     double theta, int degree, int batch_size, int leaf_size, int sm_count,
+                     int shard_rank, int shard_world) {
+    const auto t0 = std::chrono::steady_clock::now();
+    if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world)
+        throw std::invalid_argument("shard rank/world must satisfy 0 <= rank < world");
+    if (!sources) throw std::invalid_argument("sources is NULL");
+    plan_begin(p, N, targets == nullptr || targets == sources, theta, degree, batch_size, leaf_size);
+    auto lap = [&, last = t0](int stage) mutable {
+        const auto now = std::chrono::steady_clock::now();
+        p.stage_ms[stage] += std::chrono::duration<double, std::milli>(now - last).count();
+        last = now;
+    };
+    // Algorithm 3 line 1: tree of source clusters and set of target batches
+    build_tree(p.src, sources, sources + N, sources + 2 * N, N, leaf_size);
+    if (!p.shared_order) {
+        const double* t = p.same_points ? sources : targets;
+        build_tree(p.tgt, t, t + N, t + 2 * N, N, batch_size);
+    }
+    plan_set_batches(p);
+    lap(0);
+    std::vector<int64_t> b_far_evals, b_near_evals;
+    plan_lists_host(p, b_far_evals, b_near_evals);
+    lap(1);
+    plan_set_shard(p, b_far_evals, b_near_evals, shard_rank, shard_world);
+    plan_finish(p, sm_count);
     lap(3);
     p.build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
 }

@@ -65,6 +65,8 @@ struct HostPlan {
     std::vector<int64_t> far_ptr, near_ptr;
     std::vector<int32_t> far_idx, near_idx;
     int64_t far_evals = 0, near_evals = 0;
+    int lists_b0 = 0, lists_b1 = 0;  // far_idx / near_idx are filled for the batches [lists_b0, lists_b1) (the device builder
+                                     // of a sharded plan traverses only its own batches; far_ptr / near_ptr are always complete)
 
     // clusters that carry proxy charges ("slots")
     std::vector<int32_t> slot_of_cluster;      // -1 if never approximated
@@ -92,7 +94,8 @@ struct HostPlan {
 
     double max_dist = 0;                       // upper bound of |target - source| over all pairs (root boxes)
     double build_ms = 0;
-    double stage_ms[4] = {0, 0, 0, 0};         // tree(s), MAC traversal, proxy slots + upward items, work decomposition
+    double stage_ms[4] = {0, 0, 0, 0};         // tree(s) + batches, MAC traversal, (unused), proxy slots + work decomposition
+    bool built_on_device = false;              // tree and lists came from plan_device.cu
 };
 
 // Throws std::invalid_argument / std::bad_alloc.  targets == nullptr: targets are the sources.
@@ -101,6 +104,16 @@ struct HostPlan {
 void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
                      double theta, int degree, int batch_size, int leaf_size, int sm_count,
                      int shard_rank = 0, int shard_world = 1);
+
+// The stages build_host_plan is made of; the device builder (plan_device.cu) replaces the tree and the list
+// traversal by kernels and shares the rest.
+void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size);
+void build_tree(Tree& t, const double* x, const double* y, const double* z, int64_t n, int64_t max_leaf);   // host
+void plan_set_batches(HostPlan& p);                       // batches = leaves of the batch tree; max_dist
+void plan_lists_host(HostPlan& p, std::vector<int64_t>& b_far_evals, std::vector<int64_t>& b_near_evals);
+void plan_set_shard(HostPlan& p, const std::vector<int64_t>& b_far_evals, const std::vector<int64_t>& b_near_evals,
+                    int shard_rank, int shard_world);
+void plan_finish(HostPlan& p, int sm_count);              // slots, Chebyshev grids, upward items, work decomposition
 
 // Cut nb batches with the given costs into `world` contiguous slices of nearly equal cost:
 // slice r = [cut[r], cut[r+1]), cut[0] = 0, cut[world] = nb; every cut is the first batch whose

@@ -1,0 +1,146 @@
+"""SURVEY.md 8(f) NEXT-4a: the plan built ON THE DEVICE (plan_device.cu: tree by per-level stable radix sorts, MAC lists
+by one thread per batch) is the oracle's plan -- permutation, cluster ranges and lists integer-exact, boxes bitwise --
+on every case of tests/test_library_host.py, its fuzz, separate targets, sharded plans and the bench sizes; and the
+host builder behind the same entry point gives the same plan and bitwise the same convolution."""
+import numpy as np
+import pytest
+
+from paper_2003_01833_b200 import binding as B
+from paper_2003_01833_b200 import inputs as I
+from test_library_host import CASES
+
+pytestmark = pytest.mark.gpu
+
+
+def _dev(c_or_X, w=None):
+    import torch
+    X = c_or_X if isinstance(c_or_X, np.ndarray) else c_or_X.coords()
+    Xd = torch.from_numpy(np.ascontiguousarray(X)).cuda()
+    wd = torch.from_numpy(np.ones(X.shape[1]) if w is None else w).cuda()
+    return Xd, wd
+
+
+def _same_plan(e, oe, msg=""):
+    for key in e:                                            # integer-exact permutation/ranges/lists, bitwise boxes
+        np.testing.assert_array_equal(e[key], oe[key], err_msg=f"{msg} {key}")
+
+
+@pytest.mark.parametrize("name,make", CASES, ids=[c[0] for c in CASES])
+def test_device_plan_is_structurally_identical_to_oracle_tree(oracle_mod, name, make):
+    c = make()
+    Xd, wd = _dev(c, c.w)
+    p = B.bltc_create(None, Xd, wd, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    st = B.bltc_get_stats(p)
+    assert st["built_on_device"] == 1
+    op = oracle_mod.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    _same_plan(B.bltc_export_plan(p), op.export(), name)
+    assert (st["n_clusters"], st["n_leaves"], st["n_batches"]) == (op.n_clusters, op.n_leaves, op.n_batches)
+    assert (st["far_evals"], st["near_evals"]) == (op.far_evals, op.near_evals)
+    assert st["shared_batches"] == op.shared_batches
+    B.bltc_destroy(p)
+
+
+def test_device_plan_fuzz_against_oracle_tree(oracle_mod):
+    # the seeded sweep of test_host_plan_fuzz_against_oracle_tree: tiny N, leaf size 1, duplicates, planar, collinear
+    rng = np.random.default_rng(20030183 + 77)
+    for case in range(40):
+        N = int(rng.choice([1, 2, 3, 17, 64, 257, 1000, 2500, 4000]))
+        leaf = int(rng.choice([1, 2, 7, 32, 100, 300]))
+        batch = leaf if rng.random() < 0.6 else int(rng.choice([1, 5, 50, 200]))
+        theta = float(rng.choice([0.0, 0.3, 0.7, 0.95]))
+        degree = int(rng.integers(1, 7))
+        X = rng.random((3, N))
+        shape = rng.integers(0, 4)
+        if shape == 1:
+            X[2] = 0.25
+        elif shape == 2:
+            X[1] = X[0]; X[2] = 0.5
+        elif shape == 3 and N > 3:
+            X[:, N // 2:] = X[:, : N - N // 2]
+        X = np.ascontiguousarray(X)
+        Xd, wd = _dev(X)
+        p = B.bltc_create(None, Xd, wd, N, theta, degree, batch, leaf)
+        st = B.bltc_get_stats(p)
+        op = oracle_mod.OraclePlan((X[0], X[1], X[2]), theta, degree, leaf, batch)
+        _same_plan(B.bltc_export_plan(p), op.export(), f"case {case} N={N} leaf={leaf} batch={batch}")
+        assert (st["far_evals"], st["near_evals"]) == (op.far_evals, op.near_evals)
+        B.bltc_destroy(p)
+
+
+def test_device_plan_separate_targets_and_host_inputs(oracle_mod):
+    c = I.random_cloud(3000, seed=10, leaf_size=200, batch_size=200, degree=4)
+    rng = np.random.default_rng(12)
+    T = np.ascontiguousarray(rng.random((3, c.N)))
+    # host arrays: uploaded inside bltc_create, the plan is still built by kernels
+    p = B.bltc_create(T, c.coords(), c.w, c.N, 0.7, 4, 200, 200)
+    assert B.bltc_get_stats(p)["built_on_device"] == 1 and B.bltc_get_stats(p)["shared_batches"] == 0
+    oe = oracle_mod.OraclePlan((c.x, c.y, c.z), 0.7, 4, 200, 200, targets=(T[0], T[1], T[2])).export()
+    _same_plan(B.bltc_export_plan(p), oe)
+    B.bltc_destroy(p)
+
+
+@pytest.mark.parametrize("world", [3])
+def test_device_plan_sharded_traverses_only_its_batches_and_exports_the_whole_plan(oracle_mod, world):
+    c = I.random_cloud(20000, n_orb=2, seed=21, clustered=True, leaf_size=300, batch_size=300, degree=4)
+    Xd, wd = _dev(c, c.w)
+    op = oracle_mod.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    oe = op.export()
+    at, seen = 0, []
+    for r in range(world):
+        dp = B.bltc_create_sharded(None, Xd, wd, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, r, world)
+        hp = B.bltc_create_host_plan_sharded(None, c.coords(), None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, r, world)
+        sd, sh = B.bltc_get_stats(dp), B.bltc_get_stats(hp)
+        for key in ("n_clusters", "n_leaves", "n_batches", "n_far", "n_near", "far_evals", "near_evals",
+                    "shard_batch_begin", "shard_batch_end", "shard_targets", "shard_far_evals", "shard_near_evals",
+                    "n_proxy_clusters", "upward_pairs", "n_far_items", "n_near_items", "partial_len"):
+            assert sd[key] == sh[key], key                   # same cuts, same work decomposition as the host builder
+        assert sd["shard_batch_begin"] == at
+        at = sd["shard_batch_end"]
+        np.testing.assert_array_equal(B.bltc_get_shard_targets(dp), B.bltc_get_shard_targets(hp))
+        seen.append(B.bltc_get_shard_targets(dp))
+        _same_plan(B.bltc_export_plan(dp), oe, f"rank {r}")  # the export completes the other ranks' lists
+        B.bltc_destroy(dp); B.bltc_destroy(hp)
+    assert at == op.n_batches
+    np.testing.assert_array_equal(np.sort(np.concatenate(seen)), np.arange(c.N))
+
+
+def test_device_and_host_builders_give_bitwise_the_same_convolution():
+    import torch
+    c = I.random_cloud(30000, n_orb=3, seed=31, clustered=True, leaf_size=400, batch_size=400, degree=6)
+    Xd, wd = _dev(c, c.w)
+    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+    outs = []
+    for builder in (B.BUILDER_DEVICE, B.BUILDER_HOST):
+        p = B.bltc_create_with_builder(None, Xd, wd, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, 0, 1, builder)
+        assert B.bltc_get_stats(p)["built_on_device"] == (1 if builder == B.BUILDER_DEVICE else 0)
+        out = torch.empty((c.n_orb, c.N), dtype=torch.float64, device="cuda")
+        B.bltc_convolve(p, c.k, f, c.n_orb, out, True)
+        torch.cuda.synchronize()
+        outs.append(out.cpu().numpy())
+        B.bltc_destroy(p)
+    np.testing.assert_array_equal(outs[0], outs[1])
+
+
+@pytest.mark.parametrize("name,make,limit_ms", [
+    ("cfg3", lambda: I.config3(), 100.0),
+    ("random_8e6", lambda: I.config4(N=8000000), 300.0),
+], ids=["cfg3", "random_8e6"])
+def test_device_plan_at_bench_sizes_matches_the_host_builder_and_is_fast(name, make, limit_ms):
+    """NEXT-4a's bar: bltc_create < 100 ms on configs[3] (3.46 M points) and < 300 ms at N = 8e6 (inputs on the device,
+    best of 3 so that first-call allocations do not count), same plan as the threaded host builder."""
+    c = make()
+    Xd, wd = _dev(c, c.w)
+    best, st = None, None
+    for _ in range(3):
+        p = B.bltc_create(None, Xd, wd, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+        s = B.bltc_get_stats(p)
+        if best is None or s["create_ms"] < best:
+            best, st = s["create_ms"], s
+        e = B.bltc_export_plan(p) if _ == 2 else None
+        B.bltc_destroy(p)
+    hp = B.bltc_create_host_plan(None, c.coords(), None, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    _same_plan(e, B.bltc_export_plan(hp), name)
+    print(f"{name}: bltc_create {best:.1f} ms (tree {st['tree_ms']:.1f}, lists {st['lists_ms']:.1f}, "
+          f"decomposition {st['decomp_ms']:.1f}, upload + what_k {st['upload_ms']:.1f}); host builder "
+          f"{B.bltc_get_stats(hp)['build_ms']:.1f} ms")
+    assert best < limit_ms, (best, st)
