@@ -13,7 +13,7 @@ HEADERS = ["kernels.cuh", "gi_kernels.cuh", "fp64_math.cuh", "plan_host.hpp", "p
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall,-pthread",
-    "-shared",
+    "-shared", "-ldl",
 ]
 
 

@@ -2,6 +2,7 @@
 // device state of a plan, and the launch sequence of one convolution.  No arithmetic of the
 // method lives here; it is all in kernels.cu (device) and plan_host.cpp (tree and lists).
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
 #include <algorithm>
 #include <chrono>
@@ -24,6 +25,13 @@ using namespace bltc;
 namespace {
 
 thread_local std::string g_err;
+
+// NVTX range (tracing) around every stage of bltc_create and every phase of a convolution: a timeline
+// tool shows them by name; without one attached the calls are no-ops.
+struct Nvtx {
+    explicit Nvtx(const char* name) { nvtxRangePushA(name); }
+    ~Nvtx() { nvtxRangePop(); }
+};
 
 int fail(int code, const std::string& msg) { g_err = msg; return code; }
 
@@ -310,6 +318,7 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
         if (!hp.shared_order) BLTC_TRY_OR_FREE(pl->tgt_perm_own.upload(to_i32(hp.tgt.perm)));
     } else {
         // NEXT-4a: tree(s) and MAC lists by kernels (plan_device.cu); decisions identical to the host builder's
+        Nvtx range_build("bltc_create: device plan build");
         const auto t0 = std::chrono::steady_clock::now();
         auto ms_since = [](std::chrono::steady_clock::time_point a) {
             return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - a).count();
@@ -339,6 +348,7 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
         hp.build_ms = ms_since(t0);
     }
 
+    Nvtx range_upload("bltc_create: upload + proxy weights of w");
     const auto t0 = std::chrono::steady_clock::now();
     // tree-ordered records
     BLTC_TRY_OR_FREE(pl->src_rec.ensure((size_t)N));
@@ -546,6 +556,7 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int64_t N = hp.N;
+    Nvtx range_call(kind == kYukawa ? "bltc_convolve" : "bltc_convolve_coulomb");
 
     // host buffers are staged through device memory inside the call
     const double* d_f = f;
@@ -590,14 +601,18 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
         cudaEvent_t* ev = h->profiling ? &h->events[g * per] : nullptr;
         if (ev) BLTC_CUDA(cudaEventRecord(ev[0], st));
         // a1: gather to tree order
-        BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->src_perm.p, N, h->fsrc.p, st));
         const double* ftgt = h->fsrc.p;
-        if (!hp.shared_order && sub) {
-            BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->tgt_perm, N, h->ftgt_own.p, st));
-            ftgt = h->ftgt_own.p;
+        {
+            Nvtx range_gather("bltc_convolve: a1 gather");
+            BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->src_perm.p, N, h->fsrc.p, st));
+            if (!hp.shared_order && sub) {
+                BLTC_CUDA(launch_gather(d_f, N, o0, ot, h->tgt_perm, N, h->ftgt_own.p, st));
+                ftgt = h->ftgt_own.p;
+            }
         }
         if (ev) BLTC_CUDA(cudaEventRecord(ev[1], st));
         // a2: upward pass
+        Nvtx range_kernels("bltc_convolve: a2 upward, a3 far, a4 near, a5 epilogue");
         BLTC_CUDA(launch_upward(ot, h->up_items.p, (int)hp.up_items.size(), h->up_reduce.p,
                                 (int)hp.up_reduce.size(), h->slot_nodes.p, hp.degree, h->src_rec.p, h->fsrc.p,
                                 h->fhat.p, h->up_chunks.p, st));
@@ -677,6 +692,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
         return fail(BLTC_EINVAL, "alpha must be finite and > 0");
     }
     if (M == 0) return BLTC_OK;
+    Nvtx range_call(kind == kYukawa ? "direct_convolve" : "direct_convolve_coulomb");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int dev = 0, sms = 0;
     BLTC_CUDA(cudaGetDevice(&dev));

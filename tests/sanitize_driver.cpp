@@ -1,0 +1,83 @@
+// Built by tests/test_sanitizers.py with -fsanitize=address,undefined: the host plan builder (plan_host.cpp) and the
+// CPU oracle (oracle/*.c) on small clouds that hit the odd paths -- duplicates, planar points, leaf size 1, a second
+// (batch) tree, sharding, empty far lists.  Prints "sanitize ok"; any ASan / UBSan report makes the run fail.
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#include "../paper_2003_01833_b200/csrc/plan_host.hpp"
+
+extern "C" {
+struct oracle_plan;
+oracle_plan* oracle_plan_create(int64_t N, const double* sx, const double* sy, const double* sz, int64_t M,
+                                const double* tx, const double* ty, const double* tz, double theta, int degree,
+                                int leaf_size, int batch_size);
+void oracle_plan_destroy(oracle_plan* p);
+void oracle_plan_sizes(const oracle_plan* p, int64_t* s);
+int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const double* f_src, const double* f_tgt, double k,
+                     int subtract, int finalize, int64_t nsel, const int64_t* sel, double* out, double* parts);
+int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double* f_src, const double* f_tgt,
+                             double alpha, int subtract, int64_t nsel, const int64_t* sel, double* out, double* parts);
+int oracle_direct(int kind, int64_t M, const double* tx, const double* ty, const double* tz, const double* tf, int64_t N,
+                  const double* sx, const double* sy, const double* sz, const double* sw, const double* sf, double k,
+                  int subtract, int finalize, double* out);
+int oracle_coulomb_direct(int64_t M, const double* tx, const double* ty, const double* tz, const double* tf, int64_t N,
+                          const double* sx, const double* sy, const double* sz, const double* sw, const double* sf,
+                          double alpha, int subtract, double* out);
+}
+
+static uint64_t rng_state = 20030183;
+static double urand() {                      // splitmix64
+    uint64_t z = (rng_state += 0x9e3779b97f4a7c15ull);
+    z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+    z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+    return (double)((z ^ (z >> 31)) >> 11) / 9007199254740992.0;
+}
+
+int main() {
+    struct Case { int64_t N; int leaf, batch, degree, shape, world; double theta; };
+    const Case cases[] = {
+        {1, 1, 1, 1, 0, 1, 0.5},       {3, 1, 2, 2, 0, 2, 0.7},      {257, 7, 7, 3, 1, 3, 0.7},   {1000, 32, 5, 4, 2, 1, 0.95},
+        {2500, 100, 100, 5, 3, 4, 0.3}, {4000, 300, 300, 2, 0, 1, 0.0}, {6000, 50, 200, 3, 0, 8, 0.8},
+    };
+    for (const Case& c : cases) {
+        const int64_t N = c.N;
+        std::vector<double> X(3 * N), w(N), f(N), out(N), out2(N);
+        for (int64_t i = 0; i < 3 * N; ++i) X[i] = urand();
+        if (c.shape == 1) for (int64_t i = 0; i < N; ++i) X[2 * N + i] = 0.25;                       // planar
+        if (c.shape == 2) for (int64_t i = 0; i < N; ++i) { X[N + i] = X[i]; X[2 * N + i] = 0.5; }   // collinear
+        if (c.shape == 3) for (int64_t i = N / 2; i < N; ++i)                                        // duplicates
+            for (int d = 0; d < 3; ++d) X[d * N + i] = X[d * N + i - N / 2];
+        for (int64_t i = 0; i < N; ++i) { w[i] = urand() / (double)N; f[i] = 2.0 * urand() - 1.0; }
+        int64_t far_evals = -1, near_evals = -1;
+        for (int r = 0; r < c.world; ++r) {
+            bltc::HostPlan p;
+            bltc::build_host_plan(p, nullptr, X.data(), N, c.theta, c.degree, c.batch, c.leaf, 148, r, c.world);
+            far_evals = p.far_evals; near_evals = p.near_evals;
+        }
+        oracle_plan* op = oracle_plan_create(N, X.data(), X.data() + N, X.data() + 2 * N, 0, nullptr, nullptr, nullptr,
+                                             c.theta, c.degree, c.leaf, c.batch);
+        if (!op) { std::printf("oracle_plan_create failed\n"); return 1; }
+        int64_t s[8];
+        oracle_plan_sizes(op, s);
+        if (s[5] != far_evals || s[6] != near_evals) { std::printf("plan mismatch N=%lld\n", (long long)N); return 1; }
+        if (oracle_bltc_eval(op, 0, w.data(), f.data(), f.data(), 1.3, 1, 1, 0, nullptr, out.data(), nullptr)) return 1;
+        if (oracle_bltc_eval_coulomb(op, w.data(), f.data(), f.data(), 0.4, 1, 0, nullptr, out2.data(), nullptr)) return 1;
+        oracle_plan_destroy(op);
+        if (N <= 2500) {
+            std::vector<double> ds(N);
+            if (oracle_direct(0, N, X.data(), X.data() + N, X.data() + 2 * N, f.data(), N, X.data(), X.data() + N,
+                              X.data() + 2 * N, w.data(), f.data(), 1.3, 1, 1, ds.data())) return 1;
+            if (c.theta == 0.0 || c.N <= 3) {      // all-direct lists: the treecode is the definition
+                for (int64_t i = 0; i < N; ++i)
+                    if (std::fabs(ds[i] - out[i]) > 1e-12 * (1.0 + std::fabs(ds[i]))) { std::printf("value mismatch\n"); return 1; }
+            }
+            if (oracle_coulomb_direct(N, X.data(), X.data() + N, X.data() + 2 * N, f.data(), N, X.data(), X.data() + N,
+                                      X.data() + 2 * N, w.data(), f.data(), 0.4, 1, ds.data())) return 1;
+        }
+    }
+    std::printf("sanitize ok\n");
+    return 0;
+}
