@@ -777,8 +777,8 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
         for (int64_t t0 = 0; t0 < M;) {
             const int64_t pb = t0 / kPB, pb_end = std::min<int64_t>(M, (pb + 1) * kPB);
             const int64_t groups = (pb_end - t0 + unit - 1) / unit;
-            int g = 8;
-            if (groups < 8) { g = 1; while (2 * g <= groups) g *= 2; }
+            int g = kTileGroupsMax;
+            if (groups < kTileGroupsMax) { g = 1; while (2 * g <= groups) g *= 2; }
             int gs = 0; while ((1 << gs) < g) ++gs;
             const int64_t cnt = std::min<int64_t>((int64_t)g * unit, pb_end - t0);
             for (int s = 0; s < nsplit; ++s)

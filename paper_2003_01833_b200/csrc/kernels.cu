@@ -5,7 +5,7 @@
 //   upward_kernel(a2)      Eq. (35) right with the barycentric form Eq. (38)-(39) PAPER.md:416-421
 //   gather / pack / epilogue (a1, a5)  Eq. (18),(20),(21) PAPER.md:193-208
 //
-// Mapping (all three pair kernels): one CTA = 8 warps = one work item = (tile of targets) x (list
+// Mapping (all three pair kernels): one CTA = kPairWarps (8) warps = one work item = (tile of targets) x (list
 // segment).  A thread owns R targets in registers (R*32 per warp = one "group"); a tile has
 // 2^gshift <= 8 groups; the 8 warps are laid out as groups x S source-split ways (S = 8 >> gshift),
 // so small batches still fill every warp.  Sources / proxy points are staged in shared memory and
@@ -24,7 +24,11 @@
 namespace bltc {
 namespace {
 
-constexpr int kNearUnroll = 2, kFarUnroll = 2;     // sources / proxy points per loop trip (x R targets)
+constexpr int kNearUnroll = 2, kFarUnroll = 2;
+// resident CTAs per SM the pair kernels are compiled for: 2 x 8 warps at <= 128 registers.  Measured alternatives
+// (DESIGN.md 10): 1 x 8 warps at 255 registers (ptxas then interleaves every pair of a proxy row) and 1 x 12 warps at
+// 168 registers are within +-2 % -- the shared-memory and FP64 pipes co-limit the tile, not the dependent-issue stalls.
+constexpr int kPairCtasPerSm = kPairWarps == 8 ? 2 : 1;     // sources / proxy points per loop trip (x R targets)
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
@@ -239,16 +243,16 @@ __device__ __forceinline__ void reduce_and_store(TargetRegs<R, OT>& T, const Wor
 #pragma unroll
         for (int r = 0; r < R; ++r)
 #pragma unroll
-            for (int o = 0; o < OT; ++o) s_red[((r * OT + o) * 8 + warp) * 32 + lane] = T.acc[r][o];
+            for (int o = 0; o < OT; ++o) s_red[((r * OT + o) * kPairWarps + warp) * 32 + lane] = T.acc[r][o];
         __syncthreads();
         if (split == 0) {
-            const int G = 8 / S;
+            const int G = kPairWarps / S;
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int o = 0; o < OT; ++o) {
                     double s = T.acc[r][o];
-                    for (int q = 1; q < S; ++q) s += s_red[((r * OT + o) * 8 + warp + q * G) * 32 + lane];
+                    for (int q = 1; q < S; ++q) s += s_red[((r * OT + o) * kPairWarps + warp + q * G) * 32 + lane];
                     T.acc[r][o] = s;
                 }
         }
@@ -324,20 +328,20 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
 }
 
 template <int R, int OT, bool SUB, bool GUARD, int KIND>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
             const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
             double* __restrict__ partial, int64_t partial_len) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int RD = SrcRec<OT>::kDoubles;
-    static_assert(RD * kSrcTile >= R * OT * 8 * 32, "reduction scratch fits in the tile");
+    static_assert(RD * kSrcTile >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kPairThreads);
     double* s_tile = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
-    const int G = 1 << it.gshift, sshift = 3 - it.gshift;
+    const int G = 1 << it.gshift, S = kPairWarps >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
     TargetRegs<R, OT> T;
     load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
@@ -351,7 +355,7 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
             const Range rg = ranges[q];
             const int n = min(kSrcTile - fill, rg.end - at);
             flags |= rg.flags;
-            for (int i = tid; i < n; i += kThreads) {
+            for (int i = tid; i < n; i += kPairThreads) {
                 const double4 v = src_rec[at + i];
                 double* d = s_tile + (fill + i) * RD;
                 *reinterpret_cast<double2*>(d) = make_double2(v.x, v.y);
@@ -363,11 +367,11 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
             if (at == rg.end) { ++q; if (q < it.list_end) at = ranges[q].begin; }
         }
         __syncthreads();
-        const int j0 = (fill * split) >> sshift, j1 = (fill * (split + 1)) >> sshift;
+        const int j0 = (fill * split) / S, j1 = (fill * (split + 1)) / S;
         if (flags & kRangeMayCoincide) near_tile<R, OT, SUB, GUARD, true, KIND>(T, s_tile, j0, j1, kp, tab, mr);
         else near_tile<R, OT, SUB, GUARD, false, KIND>(T, s_tile, j0, j1, kp, tab, mr);
     }
-    reduce_and_store<R, OT>(T, it, warp, lane, split, 8 >> it.gshift, s_tile, partial, partial_len);
+    reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_tile, partial, partial_len);
 }
 
 // ------------------------------------------------------------------------------------ a3
@@ -380,7 +384,7 @@ template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 
 // KIND = kCoulomb: acc += (fhat_k - f_i what_k e^{-r^2/alpha^2}) / r  (reading R21: the Gaussian of Eq. (23)
 // is interpolated with the proxy weights of w).
 template <int R, int OT, bool SUB, bool GUARD, int KIND, int N1>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
 far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
            const double* __restrict__ slot_nodes, const double* __restrict__ what,
            const double* __restrict__ fhat, int n1_arg, const double4* __restrict__ tgt_rec,
@@ -388,17 +392,17 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
            int64_t partial_len) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PD = ProxyRec<OT>::kDoubles;
-    static_assert(kProxyTile * PD >= R * OT * 8 * 32, "reduction scratch fits in the tile");
+    static_assert(kProxyTile * PD >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
     constexpr int kU = N1 ? N1 : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kThreads);
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kPairThreads);
     double* s_pts = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     double* s_nodes = s_pts + kProxyTile * PD;           // [3][21]
     const MathRegs mr = math_regs_init(kMathOpaque);
     const ExpConst ec{kp.c1, kp.c3};
     const WorkItem it = items[blockIdx.x];
-    const int G = 1 << it.gshift, S = 8 >> it.gshift;
+    const int G = 1 << it.gshift, S = kPairWarps >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
     TargetRegs<R, OT> T;
     load_targets<R, OT, SUB>(T, it, grp, lane, tgt_rec, ftgt);
@@ -413,9 +417,9 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
             const int npts = (k1b - k1a) * plane;
             __syncthreads();
             if (k1a == 0)
-                for (int i = tid; i < 3 * n1; i += kThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
+                for (int i = tid; i < 3 * n1; i += kPairThreads) s_nodes[i] = slot_nodes[(size_t)slot * 3 * n1 + i];
             const size_t base = (size_t)slot * P + (size_t)k1a * plane;
-            for (int i = tid; i < npts; i += kThreads) {
+            for (int i = tid; i < npts; i += kPairThreads) {
                 double* d = s_pts + i * PD;
                 d[0] = SUB ? what[base + i] : 0.0;
 #pragma unroll
@@ -652,7 +656,7 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
         auto kern = K<RV, OTV, SV, GV>::get();                                                          \
         cudaError_t e = set_smem(kern, smem);                                                           \
         if (e != cudaSuccess) return e;                                                                 \
-        kern<<<grid, kThreads, smem, st>>>(args...);                                                    \
+        kern<<<grid, kPairThreads, smem, st>>>(args...);                                                    \
         return cudaGetLastError();                                                                      \
     }
 #define BLTC_SG(RV, OTV)                                                                                \

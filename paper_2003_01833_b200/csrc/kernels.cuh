@@ -8,7 +8,8 @@
 namespace bltc {
 
 constexpr int kMaxOT = 4;          // orbitals processed together in one pass (register tile)
-constexpr int kThreads = 256;      // 8 warps per CTA
+constexpr int kThreads = 256;      // 8 warps per CTA (upward pass, epilogue, utilities)
+constexpr int kPairThreads = 32 * kPairWarps;   // pair kernels (plan_host.hpp)
 constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (near field / direct)
 constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field)
 

@@ -179,14 +179,14 @@ struct Traversal {
 int ilog2_floor(int v) { int s = 0; while ((2 << s) <= v) ++s; return s; }
 
 // Tiles of a batch: binary decomposition of its target groups into tiles of 8/4/2/1 groups,
-// so every warp of an 8-warp CTA has work (S = 8 / groups source-split ways).
+// so every warp of a CTA has work (S = kPairWarps / groups source-split ways).
 void make_tiles(int64_t tb, int64_t te, int unit, std::vector<std::pair<int32_t, int32_t>>& tiles,
                 std::vector<int>& gshift) {
     tiles.clear(); gshift.clear();
     int64_t pos = tb;
     int groups = (int)((te - tb + unit - 1) / unit);
     while (groups > 0) {
-        const int g = std::min(8, 1 << ilog2_floor(groups));
+        const int g = std::min(kTileGroupsMax, 1 << ilog2_floor(groups));
         const int64_t cnt = std::min<int64_t>((int64_t)g * unit, te - pos);
         tiles.emplace_back((int32_t)pos, (int32_t)cnt);
         gshift.push_back(ilog2_floor(g));

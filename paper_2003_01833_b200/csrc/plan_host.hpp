@@ -11,6 +11,15 @@
 
 namespace bltc {
 
+// Warps of a pair-kernel CTA (near / far / direct).  A CTA is laid out as G target groups x S source-split ways,
+// G * S = kPairWarps, G a power of two <= kTileGroupsMax -- the host cuts batches into tiles accordingly.
+#ifndef BLTC_PAIR_WARPS
+#define BLTC_PAIR_WARPS 8
+#endif
+constexpr int kPairWarps = BLTC_PAIR_WARPS;
+constexpr int kTileGroupsMax = (kPairWarps % 8 == 0) ? 8 : 4;
+static_assert(kPairWarps % kTileGroupsMax == 0, "source-split ways must be an integer");
+
 struct Cluster {
     int64_t begin = 0, end = 0;      // particle range in tree order
     double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};   // minimal bounding box

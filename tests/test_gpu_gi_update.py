@@ -100,7 +100,11 @@ def test_gi_update_rejects_bad_arguments(gpu):
     a = torch.ones(10, dtype=torch.float64, device="cuda")
     res = torch.empty(4, dtype=torch.float64, device="cuda")
     with pytest.raises(B.BltcError):
-        B.bltc_gi_update(a, a, a, a.clone(), None, 2, 10, -0.5, res)      # n_prev > 0 without phi
+        B.bltc_gi_update(a, a, a, a.clone(), None, 2, 10, -0.5, torch.empty(6, dtype=torch.float64, device="cuda"))   # n_prev > 0 without phi
+    with pytest.raises(ValueError):      # the binding checks buffer sizes before the library sees the pointers
+        B.bltc_gi_update(a, a, a, a.clone(), None, 2, 10, -0.5, res)      # result needs 4 + n_prev elements
+    with pytest.raises(ValueError):
+        B.bltc_gi_update(a, a[:5].clone(), a, a.clone(), None, 0, 10, -0.5, res)
     with pytest.raises(B.BltcError):
         B.bltc_gi_update(a, a, a, a.clone(), None, 0, 0, -0.5, res)
     with pytest.raises(B.BltcError):
