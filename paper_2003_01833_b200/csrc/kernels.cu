@@ -327,20 +327,17 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
     }
 }
 
+// The work of one near-field CTA with R targets per thread (R = 2: groups of 64 targets; R = 1: the half-group tile
+// that holds a batch's last <= 32 targets, WorkItem::half).
 template <int R, int OT, bool SUB, bool GUARD, int KIND>
-__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
-near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
-            const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
-            const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
-            double* __restrict__ partial, int64_t partial_len) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__device__ __forceinline__ void near_body(const WorkItem& it, const Range* __restrict__ ranges,
+                                          const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
+                                          const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt,
+                                          const KPar& kp, double* __restrict__ partial, int64_t partial_len,
+                                          double* s_tile, uint32_t tab, const MathRegs& mr) {
     constexpr int RD = SrcRec<OT>::kDoubles;
     static_assert(RD * kSrcTile >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kPairThreads);
-    double* s_tile = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
-    const MathRegs mr = math_regs_init(kMathOpaque);
-    const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, S = kPairWarps >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
     TargetRegs<R, OT> T;
@@ -374,6 +371,21 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
     reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_tile, partial, partial_len);
 }
 
+template <int R, int OT, bool SUB, bool GUARD, int KIND>
+__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
+near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
+            const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
+            const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt, const KPar kp,
+            double* __restrict__ partial, int64_t partial_len) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, kPairThreads);
+    double* s_tile = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
+    const MathRegs mr = math_regs_init(kMathOpaque);
+    const WorkItem it = items[blockIdx.x];
+    if (it.half) near_body<1, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+    else near_body<R, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+}
+
 // ------------------------------------------------------------------------------------ a3
 // Shared-memory tile of proxy points: one record {what_k, fhat_k[OT]} per point (padded to 16 bytes),
 // k3 fastest, so a (k1, k2) row of the tensor grid is n1 consecutive records.  N1 > 0: the grid size
@@ -384,24 +396,19 @@ template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 
 // KIND = kCoulomb: acc += (fhat_k - f_i what_k e^{-r^2/alpha^2}) / r  (reading R21: the Gaussian of Eq. (23)
 // is interpolated with the proxy weights of w).
 template <int R, int OT, bool SUB, bool GUARD, int KIND, int N1>
-__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
-far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
-           const double* __restrict__ slot_nodes, const double* __restrict__ what,
-           const double* __restrict__ fhat, int n1_arg, const double4* __restrict__ tgt_rec,
-           const double* __restrict__ ftgt, const KPar kp, double* __restrict__ partial,
-           int64_t partial_len) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__device__ __forceinline__ void far_body(const WorkItem& it, const int32_t* __restrict__ far_slots,
+                                         const double* __restrict__ slot_nodes, const double* __restrict__ what,
+                                         const double* __restrict__ fhat, int n1_arg,
+                                         const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt,
+                                         const KPar& kp, double* __restrict__ partial, int64_t partial_len,
+                                         double* s_pts, uint32_t tab, const MathRegs& mr) {
     constexpr int PD = ProxyRec<OT>::kDoubles;
     static_assert(kProxyTile * PD >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
     constexpr int kU = N1 ? N1 : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), tid, kPairThreads);
-    double* s_pts = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     double* s_nodes = s_pts + kProxyTile * PD;           // [3][21]
-    const MathRegs mr = math_regs_init(kMathOpaque);
     const ExpConst ec{kp.c1, kp.c3};
-    const WorkItem it = items[blockIdx.x];
     const int G = 1 << it.gshift, S = kPairWarps >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
     TargetRegs<R, OT> T;
@@ -488,6 +495,22 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
         }
     }
     reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_pts, partial, partial_len);
+}
+
+template <int R, int OT, bool SUB, bool GUARD, int KIND, int N1>
+__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
+far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_slots,
+           const double* __restrict__ slot_nodes, const double* __restrict__ what,
+           const double* __restrict__ fhat, int n1_arg, const double4* __restrict__ tgt_rec,
+           const double* __restrict__ ftgt, const KPar kp, double* __restrict__ partial,
+           int64_t partial_len) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t tab = exp_table_init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, kPairThreads);
+    double* s_pts = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
+    const MathRegs mr = math_regs_init(kMathOpaque);
+    const WorkItem it = items[blockIdx.x];
+    if (it.half) far_body<1, OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
+    else far_body<R, OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
 }
 
 // ------------------------------------------------------------------------------------ a5

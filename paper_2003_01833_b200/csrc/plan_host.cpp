@@ -181,16 +181,24 @@ int ilog2_floor(int v) { int s = 0; while ((2 << s) <= v) ++s; return s; }
 // Tiles of a batch: binary decomposition of its target groups into tiles of 8/4/2/1 groups,
 // so every warp of a CTA has work (S = kPairWarps / groups source-split ways).
 void make_tiles(int64_t tb, int64_t te, int unit, std::vector<std::pair<int32_t, int32_t>>& tiles,
-                std::vector<int>& gshift) {
-    tiles.clear(); gshift.clear();
+                std::vector<int>& gshift, std::vector<int>& half) {
+    tiles.clear(); gshift.clear(); half.clear();
     int64_t pos = tb;
-    int groups = (int)((te - tb + unit - 1) / unit);
+    const int64_t rem = (te - tb) % unit;
+    const bool tail_half = rem > 0 && rem <= unit / 2;       // last <= 32 targets: their own one-target-per-thread tile
+    int groups = (int)((te - tb + unit - 1) / unit) - (tail_half ? 1 : 0);
     while (groups > 0) {
         const int g = std::min(kTileGroupsMax, 1 << ilog2_floor(groups));
         const int64_t cnt = std::min<int64_t>((int64_t)g * unit, te - pos);
         tiles.emplace_back((int32_t)pos, (int32_t)cnt);
         gshift.push_back(ilog2_floor(g));
+        half.push_back(0);
         pos += cnt; groups -= g;
+    }
+    if (tail_half) {
+        tiles.emplace_back((int32_t)pos, (int32_t)rem);
+        gshift.push_back(0);
+        half.push_back(1);
     }
 }
 
@@ -398,7 +406,7 @@ void plan_finish(HostPlan& p, int sm_count) {
         Chunk& K = chunks[ch];
         const int c0 = B0 + (int)((int64_t)(B1 - B0) * ch / nchunk), c1 = B0 + (int)((int64_t)(B1 - B0) * (ch + 1) / nchunk);
         std::vector<Range> r;
-        std::vector<std::pair<int32_t, int32_t>> tiles, nseg_slices, fseg_slices; std::vector<int> gsh;
+        std::vector<std::pair<int32_t, int32_t>> tiles, nseg_slices, fseg_slices; std::vector<int> gsh, hf;
         for (int b = c0; b < c1; ++b) {
             r.clear();
             for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) {
@@ -458,16 +466,16 @@ void plan_finish(HostPlan& p, int sm_count) {
             p.b_nseg_far[b] = (int32_t)fseg_slices.size();
             p.b_nseg_near[b] = (int32_t)nseg_slices.size();
             p.b_partial_base[b] = K.partial;                      // relative to the chunk
-            make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh);
+            make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh, hf);
             for (size_t ti = 0; ti < tiles.size(); ++ti) {
                 const int64_t local = tiles[ti].first - p.b_begin[b];
                 for (size_t s = 0; s < fseg_slices.size(); ++s)
                     K.far_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                        fseg_slices[s].first, fseg_slices[s].second, 0,
+                        fseg_slices[s].first, fseg_slices[s].second, hf[ti],
                         K.partial + (int64_t)s * nt + local});
                 for (size_t s = 0; s < nseg_slices.size(); ++s) {
                     K.near_items.push_back(WorkItem{tiles[ti].first, tiles[ti].second, gsh[ti],
-                        nseg_slices[s].first, nseg_slices[s].second, 0,
+                        nseg_slices[s].first, nseg_slices[s].second, hf[ti],
                         K.partial + (int64_t)(fseg_slices.size() + s) * nt + local});
                     int64_t key = 0;
                     for (int32_t q = nseg_slices[s].first; q < nseg_slices[s].second; ++q)

@@ -33,14 +33,15 @@ struct Tree {
     std::vector<int> leaves;         // leaf ids in DFS order
 };
 
-// One CTA's work: a tile of targets (groups of 64 consecutive targets, 2 per thread; 2^gshift groups)
+// One CTA's work: a tile of targets (groups of 64 consecutive targets, 2 per thread; 2^gshift groups -- or one half
+// group of <= 32, so that a ragged batch wastes at most 31 lanes instead of 63)
 // against one segment of its batch's far or near list.
 struct WorkItem {
     int32_t tgt_begin;               // first target (target tree order)
     int32_t tgt_count;               // targets in the tile
     int32_t gshift;                  // log2(number of target groups in the tile), 0..3
     int32_t list_begin, list_end;    // slice of near_ranges / far_slots
-    int32_t pad;
+    int32_t half;                    // 1: a half-group tile -- the last <= 32 targets of a batch, one target per thread
     int64_t partial_off;             // where this (batch, segment) slice starts in the partial buffer
 };
 

@@ -94,7 +94,7 @@ def check_full_size(gpu, oracle_mod, c, batches, orbitals, subtract, n_direct=60
 # ~1e-14).  north_star's 1e-6 at theta 0.7 / degree 8 is "parity unpinned" against the paper:
 # measured 3e-7 (cfg1), 2e-7 (cfg4), 1.2e-6 (cfg3, worst of 21 orbitals), 2.0e-6 (cfg2 at theta 0.6).  The
 # bounds below are regression bands around those measurements, not tuned targets.
-@pytest.mark.parametrize("theta,degree,tol", [(0.8, 6, 1e-3), (0.6, 8, 5e-6), (0.6, 6, 1e-4), (0.8, 8, 1e-4), (0.7, 8, 5e-6)])
+@pytest.mark.parametrize("theta,degree,tol", [(0.8, 6, 1e-3), (0.6, 8, 5e-6), (0.6, 6, 2e-4), (0.8, 8, 5e-5), (0.7, 8, 2e-5)])
 def test_config2_co_like(gpu, oracle_mod, theta, degree, tol):
     # BASELINE.json configs[2]: theta in {0.6, 0.8} x degree in {6, 8} -- all four -- plus the paper's (0.7, 8) at
     # which north_star states its 1e-6 method target; 7 orbitals = register tiles 4 + 3
