@@ -5,7 +5,8 @@ cube, w ~ U(0,1)/N, f ~ U(-1,1); the single-GPU analogue of PAPER.md:464-472 Fig
   python -m paper_2003_01833_b200.sweep [--quick] [--kernel yukawa|coulomb] > sweep.md
 
 For every (N, theta, degree, k) -- N in {1e6, 2e6, 8e6}, theta in {0.5, 0.7, 0.9}, degree 4..10, k in {0.5, 1, 5} -- it
-prints one markdown row: time per convolution (CUDA events, median of 3 (2 at N = 8e6) after a warm-up), equivalent interactions/s = N^2 / t, the kernel evaluations the plan performs, and the relative 2-norm error
+prints one markdown row: time per convolution (CUDA events, median of 3 (2 at N = 8e6) after a warm-up), equivalent
+interactions/s = N^2 / t, the kernel evaluations the plan performs, and the relative 2-norm error
 of bltc_convolve against direct_convolve on 1e4 seeded sampled targets (both on the GPU; the direct sum itself is
 pinned to the CPU oracle by tests/).  Subtraction is off: the points are not a quadrature.  Needs a CUDA device.
 """
