@@ -150,6 +150,9 @@ def sample_batches(n_batches, count=4):
 CPU_SAMPLE_BATCHES = 4      # both CPU legs (cpu_baseline inside the CUDA arm, --impl reference) time this sample
 
 
+_ORACLE_PLANS = {}
+
+
 def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
     """Time the CPU oracle's BLTC (as it stands) on a bounded sample of the workload -- CPU_SAMPLE_BATCHES evenly
     spread target batches, the first orbital -- and scale to the whole convolution phase by phase: the proxy-charge
@@ -160,8 +163,11 @@ def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
     -O3 -march=native -ffast-math (oracle/liboracle_fast.so; timing only, never used for parity).
     Returns (equiv. interactions/s, seconds of the sample, description, threads)."""
     import oracle
-    op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size, fast=fast)
-    e = op.export()
+    key = (c.name, c.theta, c.degree, c.leaf_size, c.batch_size, fast)
+    if key not in _ORACLE_PLANS:          # the oracle's tree + lists: built once, outside every timed sample
+        op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size, fast=fast)
+        _ORACLE_PLANS[key] = (op, op.export())
+    op, e = _ORACLE_PLANS[key]
     size = e["cl_end"] - e["cl_begin"]
     batches = sample_batches(op.n_batches, CPU_SAMPLE_BATCHES)
     ev, need = 0, set()

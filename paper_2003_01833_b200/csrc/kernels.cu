@@ -28,7 +28,7 @@ constexpr int kNearUnroll = 2, kFarUnroll = 2;
 // resident CTAs per SM the pair kernels are compiled for: 2 x 8 warps at <= 128 registers.  Measured alternatives
 // (DESIGN.md 10): 1 x 8 warps at 255 registers (ptxas then interleaves every pair of a proxy row) and 1 x 12 warps at
 // 168 registers are within +-2 % -- the shared-memory and FP64 pipes co-limit the tile, not the dependent-issue stalls.
-constexpr int kPairCtasPerSm = kPairWarps == 8 ? 2 : 1;     // sources / proxy points per loop trip (x R targets)
+constexpr int kPairCtasPerSm = (kPairWarps == 8 && kTargetsPerThread <= 2) ? 2 : 1;     // sources / proxy points per loop trip (x R targets)
 
 constexpr double kInv2Pi = 0.15915494309189533577;   // 2 / (4 pi)
 
@@ -328,7 +328,7 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
 }
 
 // The work of one near-field CTA with R targets per thread (R = 2: groups of 64 targets; R = 1: the half-group tile
-// that holds a batch's last <= 32 targets, WorkItem::half).
+// tiles that hold the tail of a ragged batch, WorkItem::rshift).
 template <int R, int OT, bool SUB, bool GUARD, int KIND>
 __device__ __forceinline__ void near_body(const WorkItem& it, const Range* __restrict__ ranges,
                                           const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
@@ -382,8 +382,13 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
     double* s_tile = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
-    if (it.half) near_body<1, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
-    else near_body<R, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+    if (it.rshift == 0) {
+        near_body<R, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+    } else if (R >= 4 && it.rshift == 2) {
+        near_body<(R >= 4 ? R / 4 : 1), OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+    } else {
+        near_body<(R >= 2 ? R / 2 : 1), OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+    }
 }
 
 // ------------------------------------------------------------------------------------ a3
@@ -509,8 +514,13 @@ far_kernel(const WorkItem* __restrict__ items, const int32_t* __restrict__ far_s
     double* s_pts = reinterpret_cast<double*>(smem_raw + kExpTableSmemBytes);
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
-    if (it.half) far_body<1, OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
-    else far_body<R, OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
+    if (it.rshift == 0) {
+        far_body<R, OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
+    } else if (R >= 4 && it.rshift == 2) {
+        far_body<(R >= 4 ? R / 4 : 1), OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
+    } else {
+        far_body<(R >= 2 ? R / 2 : 1), OT, SUB, GUARD, KIND, N1>(it, far_slots, slot_nodes, what, fhat, n1_arg, tgt_rec, ftgt, kp, partial, partial_len, s_pts, tab, mr);
+    }
 }
 
 // ------------------------------------------------------------------------------------ a5
@@ -671,7 +681,7 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
     return cudaGetLastError();
 }
 
-// kernel<R, OT, SUB, GUARD> dispatch on (ot, subtract, guard); R = kTargetsPerThread = 2
+// kernel<R, OT, SUB, GUARD> dispatch on (ot, subtract, guard); R = kTargetsPerThread
 template <template <int, int, bool, bool> class K, typename... Args>
 cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int grid, cudaStream_t st, Args... args) {
 #define BLTC_GO(RV, OTV, SV, GV)                                                                        \
@@ -686,10 +696,10 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
     if (subtract) { if (guard) BLTC_GO(RV, OTV, true, true) else BLTC_GO(RV, OTV, true, false) }        \
     else { if (guard) BLTC_GO(RV, OTV, false, true) else BLTC_GO(RV, OTV, false, false) }
     switch (ot) {
-        case 1: BLTC_SG(2, 1)
-        case 2: BLTC_SG(2, 2)
-        case 3: BLTC_SG(2, 3)
-        case 4: BLTC_SG(2, 4)
+        case 1: BLTC_SG(kTargetsPerThread, 1)
+        case 2: BLTC_SG(kTargetsPerThread, 2)
+        case 3: BLTC_SG(kTargetsPerThread, 3)
+        case 4: BLTC_SG(kTargetsPerThread, 4)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_SG

@@ -13,9 +13,8 @@ constexpr int kPairThreads = 32 * kPairWarps;   // pair kernels (plan_host.hpp)
 constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (near field / direct)
 constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field)
 
-// targets per thread (register tile R x OT): R = 2 for every orbital-tile width -- one staged source / proxy
-// record feeds two pair evaluations (measured on B200, profiles/r02a: near -8 %, far -2 % at OT = 4 against R = 1)
-constexpr int kTargetsPerThread = 2;
+// kTargetsPerThread (plan_host.hpp): targets per thread of a full tile, R = 2 for every orbital-tile width -- one staged
+// source / proxy record feeds two pair evaluations (measured on B200: near -8 %, far -2 % at OT = 4 against R = 1)
 
 // per-orbital constants of the tile (kernel parameter -> constant bank):
 //   nk = -k_o;  c = -k_o T/ln2 (scaled exponent argument of fp64_math.cuh's exp);  c1, c3: polynomial

@@ -180,25 +180,35 @@ int ilog2_floor(int v) { int s = 0; while ((2 << s) <= v) ++s; return s; }
 
 // Tiles of a batch: binary decomposition of its target groups into tiles of 8/4/2/1 groups,
 // so every warp of a CTA has work (S = kPairWarps / groups source-split ways).
-void make_tiles(int64_t tb, int64_t te, int unit, std::vector<std::pair<int32_t, int32_t>>& tiles,
-                std::vector<int>& gshift, std::vector<int>& half) {
-    tiles.clear(); gshift.clear(); half.clear();
+void make_tiles(int64_t tb, int64_t te, std::vector<std::pair<int32_t, int32_t>>& tiles,
+                std::vector<int>& gshift, std::vector<int>& rshift) {
+    tiles.clear(); gshift.clear(); rshift.clear();
+    constexpr int unit = 32 * kTargetsPerThread;
+    // The ragged tail (rem < unit targets) is covered by single narrower groups of 32 (R >> rs) targets, the widest
+    // first, so that fewer than 32 lanes are wasted; a tail that needs the full width anyway is just the last
+    // (partial) group of the regular tiles.
+    const int64_t rem0 = (te - tb) % unit;
     int64_t pos = tb;
-    const int64_t rem = (te - tb) % unit;
-    const bool tail_half = rem > 0 && rem <= unit / 2;       // last <= 32 targets: their own one-target-per-thread tile
-    int groups = (int)((te - tb + unit - 1) / unit) - (tail_half ? 1 : 0);
+    int groups = (int)((te - tb) / unit) + ((rem0 > unit - 32) ? 1 : 0);      // full groups (+ a tail wasting < 32 lanes)
     while (groups > 0) {
         const int g = std::min(kTileGroupsMax, 1 << ilog2_floor(groups));
         const int64_t cnt = std::min<int64_t>((int64_t)g * unit, te - pos);
         tiles.emplace_back((int32_t)pos, (int32_t)cnt);
         gshift.push_back(ilog2_floor(g));
-        half.push_back(0);
+        rshift.push_back(0);
         pos += cnt; groups -= g;
     }
-    if (tail_half) {
-        tiles.emplace_back((int32_t)pos, (int32_t)rem);
+    int64_t rem = te - pos;
+    while (rem > 0) {
+        int rs = 0;                                               // narrowest group that still holds rem
+        while ((kTargetsPerThread >> (rs + 1)) >= 1 && (int64_t)(unit >> (rs + 1)) >= rem) ++rs;
+        int64_t cap = unit >> rs;
+        if (cap - rem >= 32 && (kTargetsPerThread >> (rs + 1)) >= 1) { ++rs; cap = unit >> rs; }   // fill a narrower one first
+        const int64_t cnt = std::min(cap, rem);
+        tiles.emplace_back((int32_t)pos, (int32_t)cnt);
         gshift.push_back(0);
-        half.push_back(1);
+        rshift.push_back(rs);
+        pos += cnt; rem -= cnt;
     }
 }
 
@@ -387,7 +397,7 @@ void plan_finish(HostPlan& p, int sm_count) {
     for (int b = B0; b < B1; ++b) {
         for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q)
             near_src[b] += p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin;
-        const double groups = (double)((p.b_end[b] - p.b_begin[b] + 63) / 64);
+        const double groups = (double)((p.b_end[b] - p.b_begin[b] + 63) / 64);      // cost unit: 64 targets x 1 source
         near_cost += groups * (double)near_src[b];
         far_cost += groups * (double)(p.far_ptr[b + 1] - p.far_ptr[b]) * p.P;
     }
@@ -466,7 +476,7 @@ void plan_finish(HostPlan& p, int sm_count) {
             p.b_nseg_far[b] = (int32_t)fseg_slices.size();
             p.b_nseg_near[b] = (int32_t)nseg_slices.size();
             p.b_partial_base[b] = K.partial;                      // relative to the chunk
-            make_tiles(p.b_begin[b], p.b_end[b], 64, tiles, gsh, hf);
+            make_tiles(p.b_begin[b], p.b_end[b], tiles, gsh, hf);
             for (size_t ti = 0; ti < tiles.size(); ++ti) {
                 const int64_t local = tiles[ti].first - p.b_begin[b];
                 for (size_t s = 0; s < fseg_slices.size(); ++s)

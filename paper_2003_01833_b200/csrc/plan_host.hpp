@@ -17,6 +17,12 @@ namespace bltc {
 #define BLTC_PAIR_WARPS 8
 #endif
 constexpr int kPairWarps = BLTC_PAIR_WARPS;
+// Targets per thread of a full pair-kernel tile (register tile R x OT): a target group is 32 * R consecutive targets.
+#ifndef BLTC_TARGETS_PER_THREAD
+#define BLTC_TARGETS_PER_THREAD 2
+#endif
+constexpr int kTargetsPerThread = BLTC_TARGETS_PER_THREAD;
+static_assert(kTargetsPerThread == 1 || kTargetsPerThread == 2 || kTargetsPerThread == 4, "R is 1, 2 or 4");
 constexpr int kTileGroupsMax = (kPairWarps % 8 == 0) ? 8 : 4;
 static_assert(kPairWarps % kTileGroupsMax == 0, "source-split ways must be an integer");
 
@@ -33,15 +39,16 @@ struct Tree {
     std::vector<int> leaves;         // leaf ids in DFS order
 };
 
-// One CTA's work: a tile of targets (groups of 64 consecutive targets, 2 per thread; 2^gshift groups -- or one half
-// group of <= 32, so that a ragged batch wastes at most 31 lanes instead of 63)
+// One CTA's work: a tile of targets (2^gshift groups of 32 R consecutive targets, R per thread -- or ONE narrower group
+// of 32 (R >> rshift), so that a ragged batch wastes at most 31 lanes)
 // against one segment of its batch's far or near list.
 struct WorkItem {
     int32_t tgt_begin;               // first target (target tree order)
     int32_t tgt_count;               // targets in the tile
     int32_t gshift;                  // log2(number of target groups in the tile), 0..3
     int32_t list_begin, list_end;    // slice of near_ranges / far_slots
-    int32_t half;                    // 1: a half-group tile -- the last <= 32 targets of a batch, one target per thread
+    int32_t rshift;                  // the tile runs R >> rshift targets per thread: 0 = full groups of 32 R targets;
+                                     // > 0: one narrower group holding the tail of a ragged batch
     int64_t partial_off;             // where this (batch, segment) slice starts in the partial buffer
 };
 

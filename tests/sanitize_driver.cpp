@@ -1,6 +1,6 @@
 // Built by tests/test_sanitizers.py with -fsanitize=address,undefined: the host plan builder (plan_host.cpp) and the
 // CPU oracle (oracle/*.c) on small clouds that hit the odd paths -- duplicates, planar points, leaf size 1, a second
-// (batch) tree, sharding, empty far lists.  Prints "sanitize ok"; any ASan / UBSan report makes the run fail.
+// (batch) tree, sharding, empty far lists; the work decomposition's invariants are checked on the way.  Prints "sanitize ok"; any ASan / UBSan report makes the run fail.
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -26,6 +26,44 @@ int oracle_direct(int kind, int64_t M, const double* tx, const double* ty, const
 int oracle_coulomb_direct(int64_t M, const double* tx, const double* ty, const double* tz, const double* tf, int64_t N,
                           const double* sx, const double* sy, const double* sz, const double* sw, const double* sf,
                           double alpha, int subtract, double* out);
+}
+
+// Invariants of the B200 work decomposition (plan_host.cpp plan_finish): for every batch and every list segment the
+// tiles cover each target exactly once, a tile is 2^gshift full groups (or one narrower tail group), every item's list
+// slice is valid, and the items' slices of the partial-sum buffer are disjoint and fill [0, partial_len).
+static bool check_decomposition(const bltc::HostPlan& p) {
+    using namespace bltc;
+    std::vector<char> used((size_t)p.partial_len, 0);
+    auto check_items = [&](const std::vector<WorkItem>& items, size_t list_size) {
+        for (const WorkItem& w : items) {
+            if (w.list_begin < 0 || w.list_end > (int32_t)list_size || w.list_begin >= w.list_end) return false;
+            if (w.gshift < 0 || (1 << w.gshift) > kTileGroupsMax || w.rshift < 0 || (kTargetsPerThread >> w.rshift) < 1) return false;
+            const int cap = 32 * (kTargetsPerThread >> w.rshift) << w.gshift;
+            if (w.tgt_count < 1 || w.tgt_count > cap) return false;
+            if (w.rshift > 0 && w.gshift != 0) return false;
+            if (w.gshift > 0 && w.tgt_count <= cap / 2) return false;            // no empty groups in a tile
+            if (w.partial_off < 0 || w.partial_off + w.tgt_count > p.partial_len) return false;
+            for (int32_t i = 0; i < w.tgt_count; ++i) {
+                if (used[(size_t)w.partial_off + i]) return false;                // slices are disjoint
+                used[(size_t)w.partial_off + i] = 1;
+            }
+        }
+        return true;
+    };
+    if (!check_items(p.far_items, p.far_slots.size()) || !check_items(p.near_items, p.near_ranges.size())) return false;
+    for (char u : used) if (!u) return false;                                     // ... and cover the buffer
+    int64_t expect = 0;
+    for (int b = p.shard_b0; b < p.shard_b1; ++b) {
+        if (p.b_partial_base[b] != expect) return false;
+        expect += (int64_t)(p.b_nseg_far[b] + p.b_nseg_near[b]) * (p.b_end[b] - p.b_begin[b]);
+    }
+    if (expect != p.partial_len) return false;
+    // near segments of a batch: their ranges add up to the batch's near sources, each source once
+    int64_t near_src = 0, listed = 0;
+    for (const Range& r : p.near_ranges) { if (r.end <= r.begin) return false; near_src += r.end - r.begin; }
+    for (int b = p.shard_b0; b < p.shard_b1; ++b)
+        for (int64_t q = p.near_ptr[b]; q < p.near_ptr[b + 1]; ++q) listed += p.src.cl[p.near_idx[q]].end - p.src.cl[p.near_idx[q]].begin;
+    return near_src == listed && (int64_t)p.far_slots.size() == p.far_ptr[p.shard_b1] - p.far_ptr[p.shard_b0];
 }
 
 static uint64_t rng_state = 20030183;
@@ -56,6 +94,7 @@ int main() {
             bltc::HostPlan p;
             bltc::build_host_plan(p, nullptr, X.data(), N, c.theta, c.degree, c.batch, c.leaf, 148, r, c.world);
             far_evals = p.far_evals; near_evals = p.near_evals;
+            if (!check_decomposition(p)) { std::printf("work decomposition invariant broken, N=%lld rank %d\n", (long long)N, r); return 1; }
         }
         oracle_plan* op = oracle_plan_create(N, X.data(), X.data() + N, X.data() + 2 * N, 0, nullptr, nullptr, nullptr,
                                              c.theta, c.degree, c.leaf, c.batch);
