@@ -191,6 +191,8 @@ typedef struct oracle_plan {
     int64_t *far_ptr, *near_ptr;    /* CSR offsets [nbatch+1] */
     double* nodes;                  /* [ncl][3][n+1], Eq. (37) mapped to the box */
     int64_t far_evals, near_evals;
+    int upward_mode;                /* 0: proxy charges from the cluster's own particles (reading R9, the default);
+                                       1: parents from their children (reading R23) */
 } oracle_plan;
 
 static double box_radius(const double* lo, const double* hi)
@@ -374,11 +376,102 @@ static void proxy_charges(const oracle_plan* p, int c, const double* q_caller, d
     free(acc); free(L);
 }
 
-/* Exposed for the pins: proxy charges and nodes of one cluster. */
+/* ------------------------------------------------------------------ child -> parent upward pass
+ * SURVEY.md 8(f) NEXT-4 (a variant the paper does not spell out: Alg. 3 line 2 only says "computes the approximation
+ * weights for each source cluster").  Reading R23: the proxy charges of a LEAF come from
+ * its particles, Eq. (35) right; those of an INTERNAL cluster P are the same formula applied to its children's
+ * proxy points carrying the children's proxy charges,
+ *     qhat^P_K = sum over children c, sum over k'  L^P_K1(s^c_k1') L^P_K2(s^c_k2') L^P_K3(s^c_k3')  qhat^c_k'
+ * (L^P = the barycentric basis of P's grid, Eq. (38)-(39), with the node-hit rule R7: children share box faces with
+ * their parent, so endpoint nodes do coincide).  In exact arithmetic this gives the SAME charges as Eq. (35) applied
+ * to P's own particles: sum_k' L^P_K(s^c_k') L^c_k'(y) is the degree-n interpolant of the degree-n polynomial L^P_K,
+ * i.e. L^P_K(y) itself.  Only the rounding differs (and the cost: O(N P) instead of O(N P depth)).
+ * A child whose box is degenerate on an axis (R8) has no grid; a parent with such a child takes its charges from
+ * its own particles instead. */
+void oracle_plan_set_upward(oracle_plan* p, int mode) { if (p) p->upward_mode = mode ? 1 : 0; }
+
+static int box_is_flat(const cluster_t* C)
+{
+    return C->hi[0] == C->lo[0] || C->hi[1] == C->lo[1] || C->hi[2] == C->lo[2];
+}
+
+static int from_children(const oracle_plan* p, int c)
+{
+    const cluster_t* C = &p->src.cl[c];
+    if (!p->upward_mode || C->nchild == 0) return 0;
+    for (int q = 0; q < C->nchild; ++q) if (box_is_flat(&p->src.cl[C->child[q]])) return 0;
+    return 1;
+}
+
+static void charges_from_children(const oracle_plan* p, int c, double* const* qall, double* qhat)
+{
+    int n = p->degree, n1 = n + 1, P = p->P;
+    const cluster_t* C = &p->src.cl[c];
+    const double* sP = p->nodes + (size_t)c * 3 * n1;
+    long double* acc = (long double*)calloc((size_t)P, sizeof(long double));
+    double* L = (double*)malloc((size_t)3 * n1 * n1 * sizeof(double));     /* L[d][k'][K] = L^P_K(s^c_{d,k'}) */
+    for (int q = 0; q < C->nchild; ++q) {
+        int ch = C->child[q];
+        const double* sC = p->nodes + (size_t)ch * 3 * n1;
+        const double* qc = qall[ch];
+        for (int d = 0; d < 3; ++d)
+            for (int kp = 0; kp < n1; ++kp)
+                lagrange_row(n, sP + d * n1, sC[d * n1 + kp], L + ((size_t)d * n1 + kp) * n1);
+        for (int a1 = 0; a1 < n1; ++a1)
+            for (int a2 = 0; a2 < n1; ++a2)
+                for (int a3 = 0; a3 < n1; ++a3) {
+                    double qk = qc[(a1 * n1 + a2) * n1 + a3];
+                    const double* L1 = L + ((size_t)0 * n1 + a1) * n1;
+                    const double* L2 = L + ((size_t)1 * n1 + a2) * n1;
+                    const double* L3 = L + ((size_t)2 * n1 + a3) * n1;
+                    for (int k1 = 0; k1 < n1; ++k1)
+                        for (int k2 = 0; k2 < n1; ++k2)
+                            for (int k3 = 0; k3 < n1; ++k3)
+                                acc[(k1 * n1 + k2) * n1 + k3] += (long double)(L1[k1] * L2[k2] * L3[k3] * qk);
+                }
+    }
+    for (int k = 0; k < P; ++k) qhat[k] = (double)acc[k];
+    free(acc); free(L);
+}
+
+/* Proxy charges of every cluster with need[c] != 0, in the plan's upward mode: out[c] = malloc'd double[P] (caller
+ * frees all non-NULL entries; mode 1 also leaves the descendants it had to compute).  Levels are processed deepest
+ * first; clusters of one level are independent. */
+static void proxy_charges_needed(const oracle_plan* p, const char* need, const double* q_caller, double** out)
+{
+    int ncl = p->src.ncl, P = p->P;
+    char* use = (char*)calloc((size_t)ncl, 1);
+    int maxlevel = 0;
+    for (int c = 0; c < ncl; ++c) {                         /* pre-order: parents before children */
+        if (need[c]) use[c] = 1;
+        if (use[c] && from_children(p, c))
+            for (int q = 0; q < p->src.cl[c].nchild; ++q) use[p->src.cl[c].child[q]] = 1;
+        if (p->src.cl[c].level > maxlevel) maxlevel = p->src.cl[c].level;
+    }
+    for (int level = maxlevel; level >= 0; --level) {
+        int c;
+#pragma omp parallel for schedule(dynamic, 1)
+        for (c = 0; c < ncl; ++c) {
+            if (!use[c] || p->src.cl[c].level != level) continue;
+            out[c] = (double*)malloc((size_t)P * sizeof(double));
+            if (from_children(p, c)) charges_from_children(p, c, out, out[c]);
+            else proxy_charges(p, c, q_caller, out[c]);
+        }
+    }
+    free(use);
+}
+
+/* Exposed for the pins: proxy charges (in the plan's upward mode) and nodes of one cluster. */
 int oracle_plan_proxy(const oracle_plan* p, int c, const double* q_caller, double* qhat, double* nodes3)
 {
     if (c < 0 || c >= p->src.ncl) return -1;
-    proxy_charges(p, c, q_caller, qhat);
+    char* need = (char*)calloc((size_t)p->src.ncl, 1);
+    double** all = (double**)calloc((size_t)p->src.ncl, sizeof(double*));
+    need[c] = 1;
+    proxy_charges_needed(p, need, q_caller, all);
+    memcpy(qhat, all[c], (size_t)p->P * sizeof(double));
+    for (int i = 0; i < p->src.ncl; ++i) free(all[i]);
+    free(all); free(need);
     if (nodes3) memcpy(nodes3, p->nodes + (size_t)c * 3 * (p->degree + 1), (size_t)3 * (p->degree + 1) * sizeof(double));
     return 0;
 }
@@ -403,7 +496,7 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
     if (!p || !w || !f_src || !out) return -1;
     if (subtract && !f_tgt) return -1;
     if (kind == 0 && !(k > 0.0)) return -1;
-    int n1 = p->degree + 1, P = p->P, ncl = p->src.ncl;
+    int n1 = p->degree + 1, ncl = p->src.ncl;
     int64_t nb = sel ? nsel : p->nbatch;
     /* line 2: approximation weights, for the clusters the selected batches approximate */
     char* need = (char*)calloc((size_t)ncl, 1);
@@ -418,13 +511,8 @@ int oracle_bltc_eval(const oracle_plan* p, int kind, const double* w, const doub
     for (int64_t j = 0; j < p->N; ++j) fw[j] = f_src[j] * w[j];
     int c;
     double t_phase0 = omp_get_wtime();
-#pragma omp parallel for schedule(dynamic, 1)
-    for (c = 0; c < ncl; ++c) {
-        if (!need[c]) continue;
-        fhat[c] = (double*)malloc((size_t)P * sizeof(double));
-        proxy_charges(p, c, fw, fhat[c]);
-        if (subtract) { what[c] = (double*)malloc((size_t)P * sizeof(double)); proxy_charges(p, c, w, what[c]); }
-    }
+    proxy_charges_needed(p, need, fw, fhat);
+    if (subtract) proxy_charges_needed(p, need, w, what);
     /* line 3: for each target batch, the recorded batch-cluster interactions */
     /* Targets are independent (each one's sums are accumulated by one thread, in the order written below), so the
      * threads share the flat list of the selected batches' targets -- a sample of a few batches keeps every core busy. */
@@ -506,7 +594,7 @@ int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double
 {
     if (!p || !w || !f_src || !out) return -1;
     if (subtract && (!f_tgt || !(alpha > 0.0))) return -1;
-    int n1 = p->degree + 1, P = p->P, ncl = p->src.ncl;
+    int n1 = p->degree + 1, ncl = p->src.ncl;
     int64_t nb = sel ? nsel : p->nbatch;
     char* need = (char*)calloc((size_t)ncl, 1);
     for (int64_t s = 0; s < nb; ++s) {
@@ -520,13 +608,8 @@ int oracle_bltc_eval_coulomb(const oracle_plan* p, const double* w, const double
     for (int64_t j = 0; j < p->N; ++j) fw[j] = f_src[j] * w[j];
     int c;
     double t_phase0 = omp_get_wtime();
-#pragma omp parallel for schedule(dynamic, 1)
-    for (c = 0; c < ncl; ++c) {
-        if (!need[c]) continue;
-        fhat[c] = (double*)malloc((size_t)P * sizeof(double));
-        proxy_charges(p, c, fw, fhat[c]);
-        if (subtract) { what[c] = (double*)malloc((size_t)P * sizeof(double)); proxy_charges(p, c, w, what[c]); }
-    }
+    proxy_charges_needed(p, need, fw, fhat);
+    if (subtract) proxy_charges_needed(p, need, w, what);
     /* Targets are independent (each one's sums are accumulated by one thread, in the order written below), so the
      * threads share the flat list of the selected batches' targets -- a sample of a few batches keeps every core busy. */
     int64_t ntg = 0, u;

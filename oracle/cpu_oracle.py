@@ -60,6 +60,7 @@ def _load(fast: bool = False):
     lib.oracle_plan_create.argtypes = [C.c_int64, _dp, _dp, _dp, C.c_int64, _dp, _dp, _dp,
                                        C.c_double, C.c_int, C.c_int, C.c_int]
     lib.oracle_plan_destroy.argtypes = [C.c_void_p]
+    lib.oracle_plan_set_upward.argtypes = [C.c_void_p, C.c_int]
     lib.oracle_plan_sizes.argtypes = [C.c_void_p, _ip64]
     lib.oracle_plan_export.argtypes = [C.c_void_p, _ip64, _ip64, _ip64, _ip64, _dp, _dp, _ip32, _ip32,
                                        _ip64, _ip64, _ip64, _ip32, _ip64, _ip32]
@@ -166,7 +167,10 @@ class OraclePlan:
     """Tree + batches + interaction lists of oracle/bltc_cpu.c (Algorithm 3 line 1 and the
     decisions of line 3), and the evaluation (lines 2-3)."""
 
-    def __init__(self, sources, theta, degree, leaf_size, batch_size, targets=None, fast=False):
+    def __init__(self, sources, theta, degree, leaf_size, batch_size, targets=None, fast=False,
+                 upward_from_children=False):
+        """upward_from_children: proxy charges of internal clusters from their children's proxy charges (reading R23,
+        SURVEY.md 8(f) NEXT-4) instead of from their own particles (reading R9, the default)."""
         lib = _load(fast)
         self._lib = lib
         self._s = [_d(a) for a in sources]
@@ -185,6 +189,8 @@ class OraclePlan:
                                          float(theta), int(degree), int(leaf_size), int(batch_size))
         if not self._h:
             raise ValueError("oracle_plan_create: bad arguments")
+        self.upward_from_children = bool(upward_from_children)
+        lib.oracle_plan_set_upward(self._h, int(self.upward_from_children))
         s = (C.c_int64 * 8)()
         lib.oracle_plan_sizes(self._h, s)
         (self.n_clusters, self.n_leaves, self.n_batches, self.n_far, self.n_near,
