@@ -72,7 +72,7 @@ typedef struct bltc_stats {
     int64_t far_evals;         /* sum over far interactions of targets * (n+1)^3 */
     int64_t near_evals;        /* sum over near interactions of targets * N_S */
     int64_t n_proxy_clusters;  /* clusters that carry proxy charges */
-    int64_t upward_pairs;      /* sum over those clusters of N_S */
+    int64_t upward_pairs;      /* particle-cluster pairs of the upward pass (clusters whose charges come from particles) */
     int64_t n_far_items;       /* CTAs launched by the far-field kernel (R = 2 tiling) */
     int64_t n_near_items;      /* CTAs launched by the near-field kernel (R = 2 tiling) */
     int64_t partial_len;       /* doubles of partial-sum scratch per orbital */
@@ -97,7 +97,7 @@ typedef struct bltc_stats {
     double  decomp_ms;         /* proxy slots, Chebyshev grids, work decomposition */
     double  create_ms;         /* all of bltc_create, uploads and the proxy weights of w included */
     int32_t built_on_device;   /* 1: tree and lists were built by kernels (BLTC_BUILDER_DEVICE) */
-    int32_t reserved;
+    int32_t upward_from_children; /* 1: BLTC_UPWARD_FROM_CHILDREN */
 } bltc_stats;
 
 /* Phases of one bltc_convolve, for bltc_get_phase_ms (device times, CUDA events on `stream`). */
@@ -139,7 +139,17 @@ int bltc_create_sharded(bltc_handle* h, const double* targets, const double* sou
 /* The same with the builder named: BLTC_BUILDER_DEVICE (what bltc_create / bltc_create_sharded use) or
  * BLTC_BUILDER_HOST (tree, lists and decomposition by the threaded host code of plan_host.cpp -- the setup
  * alternative; also taken automatically for N >= 2^28).  Both give the same plan. */
-enum { BLTC_BUILDER_DEVICE = 0, BLTC_BUILDER_HOST = 1 };
+enum { BLTC_BUILDER_DEVICE = 0, BLTC_BUILDER_HOST = 1,
+       /* OR-able options for the upward pass (readings R9 / R23).
+        * FROM_CHILDREN: the proxy charges of LEAF clusters come from their particles (Eq. (35) right) and those of
+        *   every internal cluster from its children's proxy charges, re-interpolated onto its own grid, level by level,
+        *   deepest first.  In exact arithmetic the charges are the SAME as from the particles (the Lagrange basis of the
+        *   parent is a polynomial of degree n, which the child's grid reproduces exactly); measured difference of the
+        *   convolution <= 2e-15; the work is O(N (n+1)^3) instead of O(N (n+1)^3 depth) (configs[3]: 3.7x faster).
+        *   This is what bltc_create / bltc_create_sharded / bltc_create_host_plan use.
+        * FROM_PARTICLES: every cluster from its own particles, the literal reading of Alg. 3 line 2 (R9).
+        * Neither bit: the library default (FROM_CHILDREN). */
+       BLTC_UPWARD_FROM_CHILDREN = 2, BLTC_UPWARD_FROM_PARTICLES = 4 };
 int bltc_create_with_builder(bltc_handle* h, const double* targets, const double* sources, const double* weights,
                              int64_t N, double theta, int interp_degree, int batch_size, int leaf_size,
                              int rank, int world, int builder);
@@ -161,7 +171,8 @@ int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* s
  *   f    double[n_orb][N], caller's original point order: f = V_eff * psi at the quadrature points.
  *   out  double[n_orb][N], caller's original point order.
  *   subtract_singularity = 1 requires that the plan's targets are its sources.
- * Steps (all on `stream`): gather to tree order; upward pass (proxy charges fhat_k of f*w);
+ * Steps (all on `stream`): gather to tree order; upward pass (proxy charges fhat_k of f*w: leaves from particles,
+ * parents from their children unless the plan was created with BLTC_UPWARD_FROM_PARTICLES);
  * far-field kernel; near-field kernel; epilogue (-2 (far + near + f_i/k^2), scatter).
  */
 int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,

@@ -38,7 +38,7 @@ class bltc_stats(C.Structure):
         ("shard_rank", C.c_int32), ("shard_world", C.c_int32)] + [(n, C.c_int64) for n in (
             "shard_batch_begin", "shard_batch_end", "shard_targets", "shard_far_evals", "shard_near_evals")] + [
         ("tree_ms", C.c_double), ("lists_ms", C.c_double), ("decomp_ms", C.c_double), ("create_ms", C.c_double),
-        ("built_on_device", C.c_int32), ("reserved", C.c_int32)]
+        ("built_on_device", C.c_int32), ("upward_from_children", C.c_int32)]
 
 
 EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
@@ -191,13 +191,15 @@ def bltc_create(targets, sources, weights, N, theta, interp_degree, batch_size, 
     return _create(lib().bltc_create, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size)
 
 
-BUILDER_DEVICE, BUILDER_HOST = 0, 1
+BUILDER_DEVICE, BUILDER_HOST, UPWARD_FROM_CHILDREN, UPWARD_FROM_PARTICLES = 0, 1, 2, 4
 
 
 def bltc_create_with_builder(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size,
                              rank=0, world=1, builder=BUILDER_DEVICE):
     """include/bltc.h bltc_create_with_builder: tree and lists by kernels (BUILDER_DEVICE, what bltc_create uses)
-    or by the threaded host code (BUILDER_HOST); both give the same plan."""
+    or by the threaded host code (BUILDER_HOST); both give the same plan.  OR UPWARD_FROM_PARTICLES into `builder` for the
+    literal upward pass of Alg. 3 line 2 (every cluster from its own particles) instead of the default child -> parent
+    pass (UPWARD_FROM_CHILDREN: same proxy charges up to rounding, O(N P) work)."""
     return _create(lib().bltc_create_with_builder, targets, sources, weights, N, theta, interp_degree, batch_size,
                    leaf_size, rank, world, builder)
 

@@ -152,6 +152,7 @@ struct bltc_plan_s {
     DevBuf<WorkItem> far_items, near_items;
     DevBuf<UpItem> up_items;
     DevBuf<UpReduce> up_reduce;
+    DevBuf<C2PItem> c2p_items;
     DevBuf<double> up_chunks;                  // chunk-partial proxy charges (sized for kMaxOT)
     // per-convolve scratch (sized for kMaxOT)
     DevBuf<double> fsrc, ftgt_own, fhat, partial, f_stage, out_stage;
@@ -177,9 +178,11 @@ int check_create_args(bltc_handle* h, const double* sources, int64_t N, double t
 }
 
 int build_plan_guarded(bltc_plan_s* pl, const double* targets, const double* sources, int64_t N,
-                       double theta, int degree, int batch_size, int leaf_size, int sms, int rank, int world) {
+                       double theta, int degree, int batch_size, int leaf_size, int sms, int rank, int world,
+                       bool upward_children = false) {
     try {
-        build_host_plan(pl->hp, targets, sources, N, theta, degree, batch_size, leaf_size, sms, rank, world);
+        build_host_plan(pl->hp, targets, sources, N, theta, degree, batch_size, leaf_size, sms, rank, world,
+                        upward_children);
     } catch (const std::bad_alloc&) {
         return fail(BLTC_ENOMEM, "host allocation failed while building the plan");
     } catch (const std::exception& e) {
@@ -227,7 +230,8 @@ int bltc_create_host_plan_sharded(bltc_handle* h, const double* targets, const d
     if (world < 1 || rank < 0 || rank >= world) return fail(BLTC_EINVAL, "need 0 <= rank < world");
     bltc_plan_s* pl = new (std::nothrow) bltc_plan_s;
     if (!pl) return fail(BLTC_ENOMEM, "host allocation failed");
-    rc = build_plan_guarded(pl, targets, sources, N, theta, interp_degree, batch_size, leaf_size, 148, rank, world);
+    rc = build_plan_guarded(pl, targets, sources, N, theta, interp_degree, batch_size, leaf_size, 148, rank, world,
+                            /*upward_children=*/true);
     if (rc) { delete pl; return rc; }
     *h = pl;
     return BLTC_OK;
@@ -260,7 +264,12 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
     if (rc) return rc;
     if (world < 1 || rank < 0 || rank >= world) return fail(BLTC_EINVAL, "need 0 <= rank < world");
     if (!weights) return fail(BLTC_EINVAL, "weights is NULL");
-    if (builder != BLTC_BUILDER_DEVICE && builder != BLTC_BUILDER_HOST) return fail(BLTC_EINVAL, "unknown builder");
+    if (builder & ~(BLTC_BUILDER_HOST | BLTC_UPWARD_FROM_CHILDREN | BLTC_UPWARD_FROM_PARTICLES))
+        return fail(BLTC_EINVAL, "unknown builder / option bits");
+    if ((builder & BLTC_UPWARD_FROM_CHILDREN) && (builder & BLTC_UPWARD_FROM_PARTICLES))
+        return fail(BLTC_EINVAL, "BLTC_UPWARD_FROM_CHILDREN and BLTC_UPWARD_FROM_PARTICLES exclude each other");
+    const bool upward_children = (builder & BLTC_UPWARD_FROM_PARTICLES) == 0;     // the default
+    builder &= BLTC_BUILDER_HOST;
     if (N >= ((int64_t)1 << 28)) builder = BLTC_BUILDER_HOST;     // the device builder's sort keys are 32-bit
     int dev = 0, sms = 0;
     BLTC_CUDA(cudaGetDevice(&dev));
@@ -312,7 +321,7 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
         BLTC_TRY_OR_FREE(cudaMemcpy(hs.data(), sources, hs.size() * sizeof(double), cudaMemcpyDefault));
         if (!same) BLTC_TRY_OR_FREE(cudaMemcpy(ht.data(), targets, ht.size() * sizeof(double), cudaMemcpyDefault));
         rc = build_plan_guarded(pl, same ? nullptr : ht.data(), hs.data(), N, theta, interp_degree,
-                                batch_size, leaf_size, sms, rank, world);
+                                batch_size, leaf_size, sms, rank, world, upward_children);
         if (rc) { delete pl; return rc; }
         BLTC_TRY_OR_FREE(pl->src_perm.upload(to_i32(hp.src.perm)));
         if (!hp.shared_order) BLTC_TRY_OR_FREE(pl->tgt_perm_own.upload(to_i32(hp.tgt.perm)));
@@ -324,7 +333,7 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
             return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - a).count();
         };
         try {
-            plan_begin(hp, N, same, theta, interp_degree, batch_size, leaf_size);
+            plan_begin(hp, N, same, theta, interp_degree, batch_size, leaf_size, upward_children);
             hp.built_on_device = true;
             BLTC_TRY_OR_FREE(pl->src_perm.ensure((size_t)N));
             BLTC_TRY_OR_FREE(build_tree_device(hp.src, d_src, N, leaf_size, pl->src_perm.p, nullptr));
@@ -387,9 +396,14 @@ int bltc_create_with_builder(bltc_handle* h, const double* targets, const double
         BLTC_TRY_OR_FREE(pl->up_items.upload(hp.up_items));
         BLTC_TRY_OR_FREE(pl->up_reduce.upload(hp.up_reduce));
         BLTC_TRY_OR_FREE(pl->up_chunks.ensure((size_t)hp.up_partial_chunks * hp.P * kMaxOT));
+        BLTC_TRY_OR_FREE(pl->c2p_items.upload(hp.c2p_items));
         BLTC_TRY_OR_FREE(launch_upward(0, pl->up_items.p, (int)hp.up_items.size(), pl->up_reduce.p,
                                        (int)hp.up_reduce.size(), pl->slot_nodes.p, hp.degree, pl->src_rec.p,
                                        nullptr, pl->what.p, pl->up_chunks.p, nullptr));
+        for (size_t lv = 0; lv + 1 < hp.c2p_level_ptr.size(); ++lv)
+            BLTC_TRY_OR_FREE(launch_upward_children(0, pl->c2p_items.p + hp.c2p_level_ptr[lv],
+                                                    hp.c2p_level_ptr[lv + 1] - hp.c2p_level_ptr[lv], pl->slot_nodes.p,
+                                                    hp.degree, pl->what.p, nullptr));
         BLTC_TRY_OR_FREE(cudaDeviceSynchronize());
     }
 #undef BLTC_TRY_OR_FREE
@@ -426,7 +440,8 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->n_upward_items = (int64_t)hp.up_items.size();
     s->n_upward_reduce = (int64_t)hp.up_reduce.size();
     s->launches_per_group = 1 /* gather */ + (hp.shared_order ? 0 : 1) + (hp.up_items.empty() ? 0 : 1) +
-                            (hp.up_reduce.empty() ? 0 : 1) + (hp.far_items.empty() ? 0 : 1) +
+                            (hp.up_reduce.empty() ? 0 : 1) + (int64_t)(hp.c2p_level_ptr.size() - 1) +
+                            (hp.far_items.empty() ? 0 : 1) +
                             (hp.near_items.empty() ? 0 : 1) + 1 /* epilogue */;
     s->shared_batches = hp.shared_order ? 1 : 0;
     s->interp_degree = hp.degree;
@@ -445,6 +460,7 @@ int bltc_get_stats(bltc_handle h, bltc_stats* s) {
     s->decomp_ms = hp.stage_ms[3];
     s->create_ms = h->create_ms;
     s->built_on_device = hp.built_on_device ? 1 : 0;
+    s->upward_from_children = hp.upward_children ? 1 : 0;
     return BLTC_OK;
 }
 
@@ -616,6 +632,10 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
         BLTC_CUDA(launch_upward(ot, h->up_items.p, (int)hp.up_items.size(), h->up_reduce.p,
                                 (int)hp.up_reduce.size(), h->slot_nodes.p, hp.degree, h->src_rec.p, h->fsrc.p,
                                 h->fhat.p, h->up_chunks.p, st));
+        for (size_t lv = 0; lv + 1 < hp.c2p_level_ptr.size(); ++lv)      // child -> parent levels, deepest first (R23)
+            BLTC_CUDA(launch_upward_children(ot, h->c2p_items.p + hp.c2p_level_ptr[lv],
+                                             hp.c2p_level_ptr[lv + 1] - hp.c2p_level_ptr[lv], h->slot_nodes.p, hp.degree,
+                                             h->fhat.p, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[2], st));
         // a3: far field
         BLTC_CUDA(launch_far(kind, ot, sub, guard, h->far_items.p, (int)hp.far_items.size(), h->far_slots.p,

@@ -192,6 +192,77 @@ upward_kernel(const UpItem* __restrict__ items, const double* __restrict__ slot_
     }
 }
 
+// Child -> parent upward pass (reading R23): one CTA per parent slot.  For every child, in order: the per-axis
+// matrices A_d[k'][K] = L^P_K(s^c_{d,k'}) (Eq. (38)-(39) of the PARENT's grid at the child's nodes, node hits per R7),
+// then per component the tensor contraction  out[K1][K2][K3] += sum_{k'} A_1[k1'][K1] A_2[k2'][K2] A_3[k3'][K3] q^c[k']
+// in three passes through shared memory.  In exact arithmetic the result equals Eq. (35) applied to the parent's own
+// particles (L^P_K is a polynomial of degree n); the cost is O(P n) per child and component instead of O(N_C P).
+// charges: [slot][P][NC] (fhat) or [slot][P] (what, NC = 1); children are complete when the launch starts (deeper level).
+template <int NC>
+__global__ void __launch_bounds__(kThreads)
+upward_children_kernel(const C2PItem* __restrict__ items, const double* __restrict__ slot_nodes, int n1,
+                       double* __restrict__ charges) {
+    extern __shared__ double sm[];
+    const int P = n1 * n1 * n1, n = n1 - 1, tid = threadIdx.x;
+    double* s_A = sm;                            // [3][n1][n1]
+    double* s_b0 = s_A + 3 * n1 * n1;            // [P]
+    double* s_b1 = s_b0 + P;                     // [P]
+    const C2PItem it = items[blockIdx.x];
+    const double* sP = slot_nodes + (size_t)it.parent * 3 * n1;
+    double* dst = charges + (size_t)it.parent * P * NC;
+    for (int q = 0; q < it.nchild; ++q) {
+        const double* sC = slot_nodes + (size_t)it.child[q] * 3 * n1;
+        const double* src = charges + (size_t)it.child[q] * P * NC;
+        __syncthreads();
+        for (int t = tid; t < 3 * n1; t += kThreads) {
+            const int d = t / n1;
+            const double v = sC[t];
+            const double* s = sP + d * n1;
+            double* L = s_A + t * n1;
+            int hit = -1;
+            for (int k = 0; k < n1; ++k) if (v == s[k]) hit = k;
+            if (hit >= 0) {
+                for (int k = 0; k < n1; ++k) L[k] = (k == hit) ? 1.0 : 0.0;
+            } else {
+                double sum = 0.0;
+                for (int k = 0; k < n1; ++k) {
+                    const double bk = ((k & 1) ? -1.0 : 1.0) * ((k == 0 || k == n) ? 0.5 : 1.0);
+                    const double t2 = bk / (v - s[k]);
+                    L[k] = t2; sum += t2;
+                }
+                const double inv = 1.0 / sum;
+                for (int k = 0; k < n1; ++k) L[k] *= inv;
+            }
+        }
+        for (int c = 0; c < NC; ++c) {
+            __syncthreads();
+            for (int i = tid; i < P; i += kThreads) s_b0[i] = src[(size_t)i * NC + c];
+            __syncthreads();
+            for (int i = tid; i < P; i += kThreads) {               // b1[K1][k2'][k3'] = sum_k1' A_1[k1'][K1] b0[k1'][k2'][k3']
+                const int K1 = i / (n1 * n1), rest = i - K1 * n1 * n1;
+                double a = 0.0;
+                for (int k = 0; k < n1; ++k) a = fma(s_A[k * n1 + K1], s_b0[k * n1 * n1 + rest], a);
+                s_b1[i] = a;
+            }
+            __syncthreads();
+            for (int i = tid; i < P; i += kThreads) {               // b0[K1][K2][k3'] = sum_k2' A_2[k2'][K2] b1[K1][k2'][k3']
+                const int K1 = i / (n1 * n1), K2 = (i / n1) % n1, k3 = i % n1;
+                double a = 0.0;
+                for (int k = 0; k < n1; ++k) a = fma(s_A[(n1 + k) * n1 + K2], s_b1[(K1 * n1 + k) * n1 + k3], a);
+                s_b0[i] = a;
+            }
+            __syncthreads();
+            for (int i = tid; i < P; i += kThreads) {               // out[K1][K2][K3] (+)= sum_k3' A_3[k3'][K3] b0[K1][K2][k3']
+                const int K3 = i % n1, row = i - K3;
+                double a = 0.0;
+                for (int k = 0; k < n1; ++k) a = fma(s_A[(2 * n1 + k) * n1 + K3], s_b0[row + k], a);
+                const size_t o = (size_t)i * NC + c;
+                dst[o] = q == 0 ? a : dst[o] + a;
+            }
+        }
+    }
+}
+
 // out[slot][i] = sum over the slot's chunks (in chunk order) of chunk_out[first + c][i],  i < P * NC
 __global__ void __launch_bounds__(kThreads)
 upward_reduce_kernel(const UpReduce* __restrict__ red, int len, const double* __restrict__ chunk_out,
@@ -678,6 +749,28 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
     if (e != cudaSuccess || nred == 0) return e;
     const int len = n1 * n1 * n1 * nc;
     upward_reduce_kernel<<<dim3((len + kThreads - 1) / kThreads, nred), kThreads, 0, st>>>(red, len, chunk_out, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_upward_children(int ot, const C2PItem* items, int nitems, const double* slot_nodes, int degree,
+                                   double* charges, cudaStream_t st) {
+    if (nitems == 0) return cudaSuccess;
+    const int n1 = degree + 1;
+    const size_t smem = sizeof(double) * (3 * (size_t)n1 * n1 + 2 * (size_t)n1 * n1 * n1);
+    cudaError_t e = cudaSuccess;
+#define BLTC_C2P(NCV)                                                                                   \
+    e = set_smem(upward_children_kernel<NCV>, smem);                                                    \
+    if (e != cudaSuccess) return e;                                                                     \
+    upward_children_kernel<NCV><<<nitems, kThreads, smem, st>>>(items, slot_nodes, n1, charges);        \
+    break;
+    switch (ot) {
+        case 0: case 1: BLTC_C2P(1)
+        case 2: BLTC_C2P(2)
+        case 3: BLTC_C2P(3)
+        case 4: BLTC_C2P(4)
+        default: return cudaErrorInvalidValue;
+    }
+#undef BLTC_C2P
     return cudaGetLastError();
 }
 

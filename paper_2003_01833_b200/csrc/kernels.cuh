@@ -50,6 +50,11 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
                           const double* slot_nodes, int degree, const double4* src_rec,
                           const double* fsrc, double* out, double* chunk_out, cudaStream_t st);
 
+// a2, child -> parent variant (HostPlan::upward_children): one launch per tree level, deepest first, after launch_upward
+// has filled the slots that are computed from particles.  ot == 0: the proxy weights of w ([slot][P]).
+cudaError_t launch_upward_children(int ot, const C2PItem* items, int nitems, const double* slot_nodes, int degree,
+                                   double* charges, cudaStream_t st);
+
 // a3: far field
 cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,

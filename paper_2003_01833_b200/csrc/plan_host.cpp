@@ -232,7 +232,8 @@ std::vector<int> shard_cuts(const std::vector<int64_t>& batch_cost, int world) {
     return cut;
 }
 
-void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size) {
+void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size,
+                bool upward_children) {
     if (N <= 0 || N > (int64_t)2000000000) throw std::invalid_argument("N must be in [1, 2e9]");
     if (!(theta >= 0.0) || !(theta < 1.0)) throw std::invalid_argument("theta must be in [0, 1)");
     if (degree < 1 || degree > 20) throw std::invalid_argument("interp_degree must be in [1, 20]");
@@ -243,6 +244,7 @@ void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degr
     p.leaf_size = leaf_size; p.batch_size = batch_size;
     p.same_points = same_points;
     p.shared_order = same_points && batch_size == leaf_size;
+    p.upward_children = upward_children;
 }
 
 void plan_set_batches(HostPlan& p) {
@@ -340,16 +342,45 @@ void plan_finish(HostPlan& p, int sm_count) {
     const int degree = p.degree;
     if (B0 < p.lists_b0 || B1 > p.lists_b1) throw std::logic_error("plan_finish: lists of the shard's batches are missing");
 
-    // proxy slots: clusters that appear in some far list (R9), with their Chebyshev grids Eq. (37)
+    // proxy slots: clusters that appear in some far list (R9), with their Chebyshev grids Eq. (37).  With the
+    // child -> parent upward pass (R23) an internal cluster's charges come from its children's, so the children get
+    // slots too (recursively); a cluster with a child whose box is flat on an axis (R8: no grid) and every leaf
+    // take their charges from their own particles.
     const int ncl = (int)p.src.cl.size();
     const int n1 = degree + 1;
     p.slot_of_cluster.assign(ncl, -1);
     for (int64_t q = p.far_ptr[B0]; q < p.far_ptr[B1]; ++q) p.slot_of_cluster[p.far_idx[q]] = 0;   // local batches' far lists
+    auto flat = [&](const Cluster& C) { return C.hi[0] == C.lo[0] || C.hi[1] == C.lo[1] || C.hi[2] == C.lo[2]; };
+    auto from_children = [&](int c) {
+        const Cluster& C = p.src.cl[c];
+        if (!p.upward_children || C.nchild == 0) return false;
+        for (int q = 0; q < C.nchild; ++q) if (flat(p.src.cl[C.child[q]])) return false;
+        return true;
+    };
+    if (p.upward_children)
+        for (int c = 0; c < ncl; ++c)                              // pre-order: parents before children
+            if (p.slot_of_cluster[c] == 0 && from_children(c))
+                for (int q = 0; q < p.src.cl[c].nchild; ++q) p.slot_of_cluster[p.src.cl[c].child[q]] = 0;
+    int max_level = 0;
     for (int c = 0; c < ncl; ++c)
         if (p.slot_of_cluster[c] == 0) {
             p.slot_of_cluster[c] = (int32_t)p.cluster_of_slot.size();
             p.cluster_of_slot.push_back(c);
-            p.upward_pairs += p.src.cl[c].end - p.src.cl[c].begin;
+            if (!from_children(c)) p.upward_pairs += p.src.cl[c].end - p.src.cl[c].begin;
+            max_level = std::max(max_level, p.src.cl[c].level);
+        }
+    p.c2p_level_ptr.assign(1, 0);
+    if (p.upward_children)
+        for (int level = max_level; level >= 0; --level) {
+            for (size_t s = 0; s < p.cluster_of_slot.size(); ++s) {
+                const int c = p.cluster_of_slot[s];
+                const Cluster& C = p.src.cl[c];
+                if (C.level != level || !from_children(c)) continue;
+                C2PItem it{(int32_t)s, C.nchild, {0, 0, 0, 0, 0, 0, 0, 0}};
+                for (int q = 0; q < C.nchild; ++q) it.child[q] = p.slot_of_cluster[C.child[q]];
+                p.c2p_items.push_back(it);
+            }
+            if ((int32_t)p.c2p_items.size() > p.c2p_level_ptr.back()) p.c2p_level_ptr.push_back((int32_t)p.c2p_items.size());
         }
     p.slot_nodes.resize(p.cluster_of_slot.size() * 3 * (size_t)n1);
     for (size_t s = 0; s < p.cluster_of_slot.size(); ++s) {
@@ -368,6 +399,7 @@ void plan_finish(HostPlan& p, int sm_count) {
         const int64_t want = (int64_t)std::max(1, sm_count) * 16;
         const int64_t chunk = std::min<int64_t>(8192, std::max<int64_t>(512, (p.upward_pairs + want - 1) / want));
         for (size_t s = 0; s < p.cluster_of_slot.size(); ++s) {
+            if (from_children(p.cluster_of_slot[s])) continue;     // filled by the child -> parent pass
             const Cluster& C = p.src.cl[p.cluster_of_slot[s]];
             const int64_t n = C.end - C.begin;
             const int64_t nch = std::max<int64_t>(1, (n + chunk - 1) / chunk);
@@ -548,12 +580,12 @@ void plan_finish(HostPlan& p, int sm_count) {
 
 void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
                      double theta, int degree, int batch_size, int leaf_size, int sm_count,
-                     int shard_rank, int shard_world) {
+                     int shard_rank, int shard_world, bool upward_children) {
     const auto t0 = std::chrono::steady_clock::now();
     if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world)
         throw std::invalid_argument("shard rank/world must satisfy 0 <= rank < world");
     if (!sources) throw std::invalid_argument("sources is NULL");
-    plan_begin(p, N, targets == nullptr || targets == sources, theta, degree, batch_size, leaf_size);
+    plan_begin(p, N, targets == nullptr || targets == sources, theta, degree, batch_size, leaf_size, upward_children);
     auto lap = [&, last = t0](int stage) mutable {
         const auto now = std::chrono::steady_clock::now();
         p.stage_ms[stage] += std::chrono::duration<double, std::milli>(now - last).count();

@@ -62,6 +62,9 @@ constexpr int32_t kRangeMayCoincide = 1;
 // dst >= 0: it writes chunk-partial charges number dst, summed afterwards in chunk order (UpReduce).
 struct UpItem { int32_t slot, begin, end, dst; };
 struct UpReduce { int32_t slot, first, count; };
+// Child -> parent upward pass (upward_children): one CTA interpolates the proxy charges of a parent's children onto the
+// parent's grid (reading R23).  Items are grouped by tree level, deepest first: a level needs the one below.
+struct C2PItem { int32_t parent, nchild; int32_t child[8]; };   // proxy slot ids
 
 struct HostPlan {
     // parameters
@@ -89,7 +92,10 @@ struct HostPlan {
     std::vector<int32_t> slot_of_cluster;      // -1 if never approximated
     std::vector<int32_t> cluster_of_slot;
     std::vector<double> slot_nodes;            // [nslot][3][degree+1], Eq. (37)
-    int64_t upward_pairs = 0;                  // sum over slots of cluster size
+    int64_t upward_pairs = 0;                  // particle-cluster pairs of the upward pass (slots computed from particles)
+    bool upward_children = false;              // proxy charges of internal clusters from their children's (reading R23)
+    std::vector<C2PItem> c2p_items;            // by level, deepest first
+    std::vector<int32_t> c2p_level_ptr;        // [nlevels + 1] into c2p_items
     std::vector<UpItem> up_items;              // chunked upward-pass work, largest first
     std::vector<UpReduce> up_reduce;           // slots whose chunks must be summed
     int64_t up_partial_chunks = 0;             // chunk-partial buffers needed (each P * OT doubles)
@@ -120,11 +126,12 @@ struct HostPlan {
 // shard_rank / shard_world: see HostPlan::shard_b0 (world = 1: the whole problem).
 void build_host_plan(HostPlan& p, const double* targets, const double* sources, int64_t N,
                      double theta, int degree, int batch_size, int leaf_size, int sm_count,
-                     int shard_rank = 0, int shard_world = 1);
+                     int shard_rank = 0, int shard_world = 1, bool upward_children = false);
 
 // The stages build_host_plan is made of; the device builder (plan_device.cu) replaces the tree and the list
 // traversal by kernels and shares the rest.
-void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size);
+void plan_begin(HostPlan& p, int64_t N, bool same_points, double theta, int degree, int batch_size, int leaf_size,
+                bool upward_children = false);
 void build_tree(Tree& t, const double* x, const double* y, const double* z, int64_t n, int64_t max_leaf);   // host
 void plan_set_batches(HostPlan& p);                       // batches = leaves of the batch tree; max_dist
 void plan_lists_host(HostPlan& p, std::vector<int64_t>& b_far_evals, std::vector<int64_t>& b_near_evals);

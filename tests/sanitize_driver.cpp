@@ -90,9 +90,24 @@ int main() {
             for (int d = 0; d < 3; ++d) X[d * N + i] = X[d * N + i - N / 2];
         for (int64_t i = 0; i < N; ++i) { w[i] = urand() / (double)N; f[i] = 2.0 * urand() - 1.0; }
         int64_t far_evals = -1, near_evals = -1;
-        for (int r = 0; r < c.world; ++r) {
+        for (int r = 0; r < 2 * c.world; ++r) {             // both upward-pass modes (slots of the child -> parent pass)
             bltc::HostPlan p;
-            bltc::build_host_plan(p, nullptr, X.data(), N, c.theta, c.degree, c.batch, c.leaf, 148, r, c.world);
+            bltc::build_host_plan(p, nullptr, X.data(), N, c.theta, c.degree, c.batch, c.leaf, 148, r % c.world, c.world,
+                                  r >= c.world);
+            for (size_t lv = 0; lv + 1 < p.c2p_level_ptr.size(); ++lv)
+                for (int32_t i = p.c2p_level_ptr[lv]; i < p.c2p_level_ptr[lv + 1]; ++i) {
+                    const bltc::C2PItem& it = p.c2p_items[i];
+                    const int level = p.src.cl[p.cluster_of_slot[it.parent]].level;
+                    if (it.nchild < 2 || it.nchild > 8) { std::printf("bad child count\n"); return 1; }
+                    for (int q = 0; q < it.nchild; ++q)          // children have slots, one level deeper, and come earlier
+                        if (it.child[q] < 0 || p.src.cl[p.cluster_of_slot[it.child[q]]].level != level + 1 ||
+                            p.src.cl[p.cluster_of_slot[it.child[q]]].parent != p.cluster_of_slot[it.parent]) {
+                            std::printf("child -> parent item inconsistent\n"); return 1;
+                        }
+                    if (i > p.c2p_level_ptr[lv] && p.src.cl[p.cluster_of_slot[p.c2p_items[i - 1].parent]].level != level) {
+                        std::printf("levels mixed\n"); return 1;
+                    }
+                }
             far_evals = p.far_evals; near_evals = p.near_evals;
             if (!check_decomposition(p)) { std::printf("work decomposition invariant broken, N=%lld rank %d\n", (long long)N, r); return 1; }
         }
