@@ -213,7 +213,8 @@ def config_dict(c, args, world):
             "degree": c.degree, "leaf_size": c.leaf_size, "batch_size": c.batch_size,
             "subtract_singularity": True, "l2": "flushed between timed iterations (256 MB write)",
             "parallelism": ("1 GPU" if world == 1 else
-                            f"target batches sharded over {world} ranks + all-gather of out (NCCL)" if sharded
+                            f"target batches sharded over {world} ranks + all-gather of out "
+                            f"({'fused into the epilogue over NVLink peer memory' if args.exchange == 'fused' else 'NCCL'})" if sharded
                             else f"{world} replicas (each rank its own orbitals), no collective")}
 
 
@@ -322,9 +323,14 @@ def run_cuda(args):
         f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
         out = torch.zeros((O, N), dtype=torch.float64, device="cuda")      # a sharded plan writes its slice only
         exchange = None
+        fused = None                                     # --exchange fused: results stored straight into the peers' buffers
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        if shard:    # strong scaling: rank r computes its slice of the target batches; the only exchange is the
+        if shard and args.exchange == "fused":
+            from paper_2003_01833_b200.multi_gpu import ShardedPlan
+            fused = ShardedPlan(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, fused_scatter=True)
+            plan = fused.plan
+        elif shard:  # strong scaling: rank r computes its slice of the target batches; the only exchange is the
             # all-gather of `out` that the next Green-Iteration step needs on every rank
             from paper_2003_01833_b200.multi_gpu import ShardExchange
             plan = B.bltc_create_sharded(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
@@ -335,6 +341,12 @@ def run_cuda(args):
         st = B.bltc_get_stats(plan)
 
         def convolve(f_, out_):
+            if fused is not None:                        # epilogue scatters over NVLink peer memory (symmetric memory)
+                if coulomb:
+                    fused.convolve_coulomb(f_, O, out_, True, 1.0)
+                else:
+                    fused.convolve(c.k, f_, O, out_, True)
+                return
             if coulomb:
                 B.bltc_convolve_coulomb(plan, f_, O, out_, True, 1.0)
             else:
@@ -372,8 +384,15 @@ def run_cuda(args):
             f_host = torch.from_numpy(np.ascontiguousarray(c.f)).pin_memory()
             out_host = torch.zeros((O, N), dtype=torch.float64).pin_memory()
             out_dev = torch.zeros((O, N), dtype=torch.float64, device="cuda") if exchange is not None else None
+            f_dev2 = torch.empty((O, N), dtype=torch.float64, device="cuda") if fused is not None else None
 
             def convolve_host():            # H2D(f) + a1..a5 + D2H(out) + stream sync, all inside the C call
+                if fused is not None:       # the scatter call takes device buffers: copies made here, inside the timed region
+                    f_dev2.copy_(f_host, non_blocking=True)
+                    res_ = fused.convolve_coulomb(f_dev2, O, None, True, 1.0) if coulomb else fused.convolve(c.k, f_dev2, O, None, True)
+                    out_host.copy_(res_, non_blocking=True)
+                    torch.cuda.current_stream().synchronize()
+                    return
                 if coulomb:
                     B.bltc_convolve_coulomb(plan, f_host, O, out_host, True, 1.0)
                 else:
@@ -536,6 +555,10 @@ def main():
     ap.add_argument("--shard", default="batches", choices=["replicas", "batches"],
                     help="N > 1: batches = one convolution, target batches sharded over the ranks + all-gather of out "
                          "(strong scaling, default); replicas = each rank convolves its own orbitals (weak scaling)")
+    ap.add_argument("--exchange", default="nccl", choices=["nccl", "fused"],
+                    help="N > 1, --shard batches: nccl = gather kernel + ONE all_gather_into_tensor + scatter kernel (default); "
+                         "fused = the epilogue kernel stores into every rank's buffer over NVLink peer memory "
+                         "(torch symmetric memory), no collective")
     ap.add_argument("--workload", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"],
                     help="cfg3 = BASELINE.json configs[3], the largest single-GPU config (the bench line); "
                          "others: profiling / context")

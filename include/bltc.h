@@ -33,9 +33,9 @@
  *     thread-local message.  No exceptions, no exit(); handles are independent and the library keeps no state
  *     between calls other than a stream-ordered memory pool of its own per device (staging buffers of
  *     direct_convolve / bltc_gi_update are reused, the device's default pool is not touched).
- *     A handle must not be used by two threads at once, and calls on one handle must be stream-ordered with
- *     respect to each other (the per-plan scratch -- proxy charges, partial sums, staging -- is shared by them):
- *     use one stream per handle, or make the second stream wait on the first.
+ *     A handle must not be used by two threads at once.  Calls on one handle share its scratch (proxy charges,
+ *     partial sums, staging); the library orders them itself: a convolve enqueued on another stream than the
+ *     previous one first waits (cudaStreamWaitEvent) for that one to finish.
  *   - There is no CPU fallback: every compute entry point fails with BLTC_ECUDA / BLTC_ENODEVICE
  *     if no CUDA device is usable.
  *   - Limits: 1 <= N <= 2e9 (int32 indices), 1 <= interp_degree <= 20, 0 <= theta < 1,
@@ -177,6 +177,21 @@ int bltc_create_host_plan(bltc_handle* h, const double* targets, const double* s
  */
 int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
                   int subtract_singularity, bltc_stream stream);
+
+/*
+ * bltc_convolve_scatter / bltc_convolve_coulomb_scatter: the same convolution, with the exchange of a batch-sharded
+ * run fused into the kernel that produces the result ("outputs stay sharded or one all-gather of
+ * out").  The epilogue stores every out[o][i] of this plan's targets into `out` AND into each of the n_peers <= 15
+ * buffers peer_outs[r] (HOST array of DEVICE pointers, each double[n_orb][N] in the caller's point order): the other
+ * ranks' `out` buffers, peer-mapped over NVLink (cudaIpc / CUDA symmetric memory; torch.distributed's symmetric
+ * memory gives the pointers, paper_2003_01833_b200/multi_gpu.py).  When every rank has run its call and the ranks have
+ * synchronised (a barrier on the symmetric memory), each rank's `out` holds the whole result: no separate gather,
+ * collective or scatter kernel.  All buffers must be device memory; n_peers = 0 is bltc_convolve.
+ */
+int bltc_convolve_scatter(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
+                          double* const* peer_outs, int n_peers, int subtract_singularity, bltc_stream stream);
+int bltc_convolve_coulomb_scatter(bltc_handle h, const double* f, int n_f, double* out, double* const* peer_outs,
+                                  int n_peers, int subtract_singularity, double alpha, bltc_stream stream);
 
 /*
  * direct_convolve: the definition, O(M N), no plan (Eq. (32); the "ds" column of

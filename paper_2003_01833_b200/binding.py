@@ -43,7 +43,8 @@ class bltc_stats(C.Structure):
 
 EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
             "bltc_create_with_builder",
-            "bltc_get_shard_targets", "bltc_convolve", "direct_convolve",
+            "bltc_get_shard_targets", "bltc_convolve", "direct_convolve", "bltc_convolve_scatter",
+            "bltc_convolve_coulomb_scatter",
             "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
@@ -71,6 +72,8 @@ def lib():
     L.bltc_convolve.argtypes = [vp, _dp, vp, C.c_int, vp, C.c_int, vp]
     L.direct_convolve.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, _dp, C.c_int, vp, C.c_int, vp]
     L.bltc_convolve_coulomb.argtypes = [vp, vp, C.c_int, vp, C.c_int, C.c_double, vp]
+    L.bltc_convolve_scatter.argtypes = [vp, _dp, vp, C.c_int, vp, C.POINTER(vp), C.c_int, C.c_int, vp]
+    L.bltc_convolve_coulomb_scatter.argtypes = [vp, vp, C.c_int, vp, C.POINTER(vp), C.c_int, C.c_int, C.c_double, vp]
     L.direct_convolve_coulomb.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, C.c_int, vp, C.c_int,
                                           C.c_double, vp]
     L.bltc_gi_update.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int64, C.c_double, vp, vp]
@@ -215,6 +218,35 @@ def bltc_convolve(plan, k, f, n_orb, out, subtract_singularity=True, stream=None
     n = int(n_orb) * plan.N
     _check(lib().bltc_convolve(plan._h, kk.ctypes.data_as(_dp), _ptr(f, "f", False, n), int(n_orb), _ptr(out, "out", False, n),
                                int(bool(subtract_singularity)), _stream_ptr(stream)))
+    return out
+
+
+def _peer_array(peers, n):
+    """HOST array of device pointers for the scatter calls: peers are tensors (checked for size) or raw addresses."""
+    arr = (C.c_void_p * max(len(peers), 1))()
+    for i, p in enumerate(peers):
+        arr[i] = int(p) if isinstance(p, int) else _ptr(p, f"peer_outs[{i}]", False, n)
+    return arr
+
+
+def bltc_convolve_scatter(plan, k, f, n_orb, out, peer_outs, subtract_singularity=True, stream=None):
+    """include/bltc.h bltc_convolve_scatter: the epilogue also stores into every buffer of peer_outs (tensors or raw
+    device addresses, e.g. the other ranks' symmetric-memory buffers)."""
+    kk = _karray(k, n_orb)
+    n = int(n_orb) * plan.N
+    arr = _peer_array(peer_outs, n)
+    _check(lib().bltc_convolve_scatter(plan._h, kk.ctypes.data_as(_dp), _ptr(f, "f", False, n), int(n_orb),
+                                       _ptr(out, "out", False, n), arr, len(peer_outs), int(bool(subtract_singularity)),
+                                       _stream_ptr(stream)))
+    return out
+
+
+def bltc_convolve_coulomb_scatter(plan, f, n_f, out, peer_outs, subtract_singularity=True, alpha=1.0, stream=None):
+    n = int(n_f) * plan.N
+    arr = _peer_array(peer_outs, n)
+    _check(lib().bltc_convolve_coulomb_scatter(plan._h, _ptr(f, "f", False, n), int(n_f), _ptr(out, "out", False, n), arr,
+                                               len(peer_outs), int(bool(subtract_singularity)), float(alpha),
+                                               _stream_ptr(stream)))
     return out
 
 

@@ -157,11 +157,18 @@ struct bltc_plan_s {
     // per-convolve scratch (sized for kMaxOT)
     DevBuf<double> fsrc, ftgt_own, fhat, partial, f_stage, out_stage;
     int last_ot = 0;
+    // the scratch above is shared by every call on this handle: a call on another stream waits for the previous one
+    cudaEvent_t last_done = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool has_last = false;
     // profiling
     bool profiling = false;
     std::vector<cudaEvent_t> events;     // (BLTC_NUM_PHASES + 1) per orbital group
     int events_used = 0;
-    ~bltc_plan_s() { for (cudaEvent_t e : events) cudaEventDestroy(e); }
+    ~bltc_plan_s() {
+        for (cudaEvent_t e : events) cudaEventDestroy(e);
+        if (last_done) cudaEventDestroy(last_done);
+    }
 };
 
 namespace {
@@ -555,8 +562,14 @@ namespace {
 
 // One convolution through the plan, kind = kYukawa (k: n_orb values) or kCoulomb (alpha; k unused).
 int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const double* f, int n_orb,
-                  double* out, int subtract_singularity, bltc_stream stream) {
+                  double* out, int subtract_singularity, bltc_stream stream, double* const* peers = nullptr,
+                  int n_peers = 0) {
     if (!h) return fail(BLTC_EINVAL, "handle is NULL");
+    if (n_peers < 0 || n_peers > kMaxOuts - 1) return fail(BLTC_EINVAL, "at most 15 additional destinations");
+    if (n_peers > 0 && !peers) return fail(BLTC_EINVAL, "peer destination array is NULL");
+    for (int r = 0; r < n_peers; ++r)
+        if (!peers[r]) return fail(BLTC_EINVAL, "a peer destination is NULL");
+    if (n_peers > 0 && out && !is_device_ptr(out)) return fail(BLTC_EINVAL, "bltc_convolve_scatter needs device buffers");
     if (!h->on_device) return fail(BLTC_ENODEVICE, "plan was built with bltc_create_host_plan (no device state)");
     if (!f || !out) return fail(BLTC_EINVAL, "f and out must not be NULL");
     if (n_orb < 1) return fail(BLTC_EINVAL, "n_orb must be >= 1");
@@ -573,6 +586,10 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int64_t N = hp.N;
     Nvtx range_call(kind == kYukawa ? "bltc_convolve" : "bltc_convolve_coulomb");
+    // per-plan scratch (fsrc, fhat, partial, staging) is reused by every call: order this call after the previous one
+    // even if the caller switched streams (same stream: already ordered)
+    if (!h->last_done) BLTC_CUDA(cudaEventCreateWithFlags(&h->last_done, cudaEventDisableTiming));
+    if (h->has_last && h->last_stream != st) BLTC_CUDA(cudaStreamWaitEvent(st, h->last_done, 0));
 
     // host buffers are staged through device memory inside the call
     const double* d_f = f;
@@ -647,17 +664,20 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
                               h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
         // a5: epilogue
+        OutSet outs;
+        outs.n = 1 + n_peers; outs.p[0] = d_out;
+        for (int r = 0; r < n_peers; ++r) outs.p[1 + r] = peers[r];
         BLTC_CUDA(launch_epilogue(ot, sub, hp.shard_b1 - hp.shard_b0, h->b_begin.p, h->b_count.p,
                                   h->b_partial_base.p, h->b_nseg.p, h->partial.p, hp.partial_len, ftgt, ep,
-                                  h->tgt_perm, d_out, N, o0, st));
+                                  h->tgt_perm, outs, N, o0, st));
         if (ev) { BLTC_CUDA(cudaEventRecord(ev[5], st)); h->events_used += per; }
         h->last_ot = ot;
         o0 += ot;
     }
-    if (out_on_host) {
-        BLTC_CUDA(cudaMemcpyAsync(out, d_out, (size_t)n_orb * N * sizeof(double), cudaMemcpyDeviceToHost, st));
-        BLTC_CUDA(cudaStreamSynchronize(st));
-    }
+    if (out_on_host) BLTC_CUDA(cudaMemcpyAsync(out, d_out, (size_t)n_orb * N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    BLTC_CUDA(cudaEventRecord(h->last_done, st));
+    h->last_stream = st; h->has_last = true;
+    if (out_on_host) BLTC_CUDA(cudaStreamSynchronize(st));
     return BLTC_OK;
 }
 
@@ -673,6 +693,16 @@ int bltc_convolve(bltc_handle h, const double* k, const double* f, int n_orb, do
 int bltc_convolve_coulomb(bltc_handle h, const double* f, int n_f, double* out, int subtract_singularity,
                           double alpha, bltc_stream stream) {
     return convolve_impl(h, kCoulomb, nullptr, alpha, f, n_f, out, subtract_singularity, stream);
+}
+
+int bltc_convolve_scatter(bltc_handle h, const double* k, const double* f, int n_orb, double* out,
+                          double* const* peer_outs, int n_peers, int subtract_singularity, bltc_stream stream) {
+    return convolve_impl(h, kYukawa, k, 0.0, f, n_orb, out, subtract_singularity, stream, peer_outs, n_peers);
+}
+
+int bltc_convolve_coulomb_scatter(bltc_handle h, const double* f, int n_f, double* out, double* const* peer_outs,
+                                  int n_peers, int subtract_singularity, double alpha, bltc_stream stream) {
+    return convolve_impl(h, kCoulomb, nullptr, alpha, f, n_f, out, subtract_singularity, stream, peer_outs, n_peers);
 }
 
 int bltc_direct_set_profiling(int enable) { g_direct_profiling = enable != 0; return BLTC_OK; }
@@ -850,9 +880,11 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }
+        OutSet outs;
+        outs.n = 1; outs.p[0] = d_out;
         BLTC_CUDA(launch_epilogue(ot, sub, (int)npb, t_pbb.as<int32_t>(), t_pbc.as<int32_t>(),
                                   t_pbs.as<int64_t>(), t_pbn.as<int32_t>(), t_partial.as<double>(), partial_len,
-                                  t_ftgt.as<double>(), ep, nullptr, d_out, M, o0, st));
+                                  t_ftgt.as<double>(), ep, nullptr, outs, M, o0, st));
         o0 += ot;
     }
     if (out_on_host) {

@@ -600,7 +600,7 @@ __global__ void __launch_bounds__(kThreads)
 epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__ b_count,
                 const int64_t* __restrict__ b_partial_base, const int32_t* __restrict__ b_nseg,
                 const double* __restrict__ partial, int64_t partial_len, const double* __restrict__ ftgt,
-                const EpiPar ep, const int32_t* __restrict__ perm, double* __restrict__ out, int64_t stride,
+                const EpiPar ep, const int32_t* __restrict__ perm, const OutSet outs, int64_t stride,
                 int o0) {
     const int b = blockIdx.x;
     const int begin = b_begin[b], count = b_count[b], nseg = b_nseg[b];
@@ -614,7 +614,8 @@ epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__
             for (int g = 0; g < nseg; ++g) s += partial[(int64_t)o * partial_len + base + (int64_t)g * count + l];
             double v = ep.scale * s;                               // Yukawa: -2 * S / (4 pi);  Coulomb: S
             if (SUB) v = fma(ep.coef[o], ftgt[(size_t)i * OT + o], v);   // -2 f_i/k^2 (Eq. (21)) / 2 pi alpha^2 f_i (Eq. (24))
-            out[(int64_t)(o0 + o) * stride + dst] = v;
+            // one result, every destination: the rank's own out and, when the all-gather is fused in, its peers'
+            for (int r = 0; r < outs.n; ++r) outs.p[r][(int64_t)(o0 + o) * stride + dst] = v;
         }
     }
 }
@@ -841,7 +842,7 @@ cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkI
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
                             int64_t partial_len, const double* ftgt, const EpiPar& kp, const int32_t* perm,
-                            double* out, int64_t stride, int o0, cudaStream_t st) {
+                            const OutSet& out, int64_t stride, int o0, cudaStream_t st) {
     if (nbatch == 0) return cudaSuccess;
 #define BLTC_EPI(OTV)                                                                                  \
     case OTV:                                                                                          \

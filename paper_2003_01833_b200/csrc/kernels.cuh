@@ -67,12 +67,17 @@ cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkI
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st);
 
+// destinations of the epilogue: the caller's out and, for a sharded plan whose all-gather is fused into the epilogue
+// (bltc_convolve_scatter), the peer ranks' out buffers (NVLink peer / symmetric memory); all double[n_orb][stride]
+constexpr int kMaxOuts = 16;
+struct OutSet { double* p[kMaxOuts]; int n; };
+
 // a5: out[o0+o][perm[i]] = ep.scale (far + near) + [subtract] ep.coef[o] f_i
 //     (Yukawa: -2 ( (far + near)/(4 pi) + f_i / k_o^2 );  Coulomb: far + near + 2 pi alpha^2 f_i)
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,
                             const int64_t* b_partial_base, const int32_t* b_nseg, const double* partial,
                             int64_t partial_len, const double* ftgt, const EpiPar& ep, const int32_t* perm,
-                            double* out, int64_t stride, int o0, cudaStream_t st);
+                            const OutSet& outs, int64_t stride, int o0, cudaStream_t st);
 
 // roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed
 cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStream_t st);

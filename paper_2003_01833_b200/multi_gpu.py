@@ -6,6 +6,10 @@ Green-Iteration step: its source field f = V_eff * psi_new is needed at ALL poin
 replicated), so after the convolution the ranks all-gather their slices of `out` -- O * N * 8 bytes in total per
 step, over NCCL (NVLink 5 / NVSwitch) for CUDA tensors, or gloo for CPU tensors (tests).
 
+`ShardedPlan(fused_scatter=True)` fuses that exchange into the convolution's epilogue kernel: results are stored
+straight into every rank's buffer over NVLink peer memory (torch.distributed symmetric memory provides the mappings
+and the barriers), so no separate collective runs.
+
 This module is plumbing only (torch.distributed + index bookkeeping); all arithmetic stays in the CUDA kernels.
 """
 from __future__ import annotations
@@ -86,23 +90,67 @@ class ShardExchange:
 
 
 class ShardedPlan:
-    """bltc_create_sharded + the exchange: `convolve` leaves the full out[n_orb][N] on every rank."""
+    """bltc_create_sharded + the exchange: `convolve` leaves the full out[n_orb][N] on every rank.
 
-    def __init__(self, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, group=None):
+    fused_scatter=False: convolution, then ShardExchange (gather kernel + ONE NCCL all-gather + scatter kernel).
+    fused_scatter=True:  the exchange is fused into the convolution's epilogue (bltc_convolve_scatter): every rank's
+        result buffer lives in torch.distributed symmetric memory, the epilogue kernel stores each value into its own
+        buffer and, over NVLink peer mappings, into every other rank's; a symmetric-memory barrier before (the peers
+        have consumed the previous result) and after (all stores have landed) replaces the collective.  The result is
+        the symmetric buffer itself (returned; copied into `out` if one is given).
+    """
+
+    def __init__(self, targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size, group=None,
+                 fused_scatter=False):
         import torch.distributed as dist
+        self.group = group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.N = int(N)
+        self.device = sources.device
         self.plan = B.bltc_create_sharded(targets, sources, weights, N, theta, interp_degree, batch_size, leaf_size,
                                           self.rank, self.world)
         self.stats = B.bltc_get_stats(self.plan)
-        self.exchange = ShardExchange(B.bltc_get_shard_targets(self.plan), N, sources.device, group)
+        self.fused = bool(fused_scatter)
+        self._symm = {}                      # n_orb -> (tensor, handle, peer pointers)
+        self.exchange = None if self.fused else ShardExchange(B.bltc_get_shard_targets(self.plan), N, sources.device, group)
 
-    def convolve(self, k, f, n_orb, out, subtract_singularity=True, gather=True):
-        B.bltc_convolve(self.plan, k, f, n_orb, out, subtract_singularity)
-        return self.exchange.all_gather_out(out) if gather else out
+    def _symm_out(self, n_orb):
+        """This rank's [n_orb][N] result buffer in symmetric memory and the other ranks' addresses of theirs
+        (collective on first use per n_orb)."""
+        if n_orb not in self._symm:
+            import torch
+            import torch.distributed as dist
+            import torch.distributed._symmetric_memory as symm_mem
+            t = symm_mem.empty((n_orb, self.N), dtype=torch.float64, device=self.device)
+            hdl = symm_mem.rendezvous(t, self.group if self.group is not None else dist.group.WORLD)
+            peers = [int(p) for r, p in enumerate(hdl.buffer_ptrs) if r != self.rank]
+            self._symm[n_orb] = (t, hdl, peers)
+        return self._symm[n_orb]
 
-    def convolve_coulomb(self, f, n_f, out, subtract_singularity=True, alpha=1.0, gather=True):
-        B.bltc_convolve_coulomb(self.plan, f, n_f, out, subtract_singularity, alpha)
-        return self.exchange.all_gather_out(out) if gather else out
+    def _run(self, call_plain, call_scatter, n_orb, out, gather):
+        if not self.fused:
+            call_plain(out)
+            return self.exchange.all_gather_out(out) if gather else out
+        t, hdl, peers = self._symm_out(n_orb)
+        hdl.barrier()                        # every rank has consumed the previous result
+        call_scatter(t, peers if gather else [])
+        hdl.barrier()                        # every rank's stores have landed
+        if out is not None and out.data_ptr() != t.data_ptr():
+            out.copy_(t)
+            return out
+        return t
+
+    def convolve(self, k, f, n_orb, out=None, subtract_singularity=True, gather=True):
+        return self._run(lambda o: B.bltc_convolve(self.plan, k, f, n_orb, o, subtract_singularity),
+                         lambda t, peers: B.bltc_convolve_scatter(self.plan, k, f, n_orb, t, peers, subtract_singularity),
+                         n_orb, out, gather)
+
+    def convolve_coulomb(self, f, n_f, out=None, subtract_singularity=True, alpha=1.0, gather=True):
+        return self._run(lambda o: B.bltc_convolve_coulomb(self.plan, f, n_f, o, subtract_singularity, alpha),
+                         lambda t, peers: B.bltc_convolve_coulomb_scatter(self.plan, f, n_f, t, peers,
+                                                                          subtract_singularity, alpha),
+                         n_f, out, gather)
 
     def destroy(self):
         B.bltc_destroy(self.plan)
+        self._symm.clear()

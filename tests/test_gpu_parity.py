@@ -310,3 +310,27 @@ def test_bltc_fuzz_degenerate_shapes(gpu, oracle_mod):
             assert ok.all(), (case, what, N, leaf, theta, degree, subtract, err, scale)
             worst = max(worst, float((err / np.maximum(scale, 1e-300)).max()))
     print(f"fuzz: worst relative error {worst:.2e}")
+
+
+def test_calls_on_one_handle_from_two_streams_are_ordered_by_the_library(gpu):
+    # bltc.h: the per-plan scratch is shared by every call on a handle; a convolve enqueued on another stream than the
+    # previous one waits for it.  Two back-to-back calls with different fields on two streams must give what two
+    # serial calls give, bitwise.
+    torch, B = gpu
+    c = I.random_cloud(60000, n_orb=4, seed=51, clustered=True, leaf_size=500, batch_size=500, degree=6)
+    X, w = dev(torch, c.coords()), dev(torch, c.w)
+    f1 = dev(torch, c.f)
+    f2 = dev(torch, c.f[::-1] * 1.7)
+    plan = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    ref1, ref2 = torch.empty_like(f1), torch.empty_like(f1)
+    B.bltc_convolve(plan, c.k, f1, 4, ref1, True)
+    B.bltc_convolve(plan, c.k, f2, 4, ref2, True)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        o1, o2 = torch.empty_like(f1), torch.empty_like(f1)
+        B.bltc_convolve(plan, c.k, f1, 4, o1, True, stream=s1)
+        B.bltc_convolve(plan, c.k, f2, 4, o2, True, stream=s2)      # enqueued while the first is still running
+        torch.cuda.synchronize()
+        assert torch.equal(o1, ref1) and torch.equal(o2, ref2)
+    B.bltc_destroy(plan)

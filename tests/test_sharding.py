@@ -274,3 +274,62 @@ def test_gpu_sharded_plan_with_nccl_world1_equals_plain_convolve():
         sp.destroy(); B.bltc_destroy(plan)
     finally:
         dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_gpu_scatter_epilogue_writes_every_destination():
+    # bltc_convolve_scatter: the epilogue stores each result into `out` and into every peer buffer (here: more buffers
+    # on the same GPU stand in for the peers' NVLink-mapped ones); a sharded plan still writes only its own targets
+    import torch
+    c = _cloud()
+    X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+    f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+    full = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    ref = torch.empty((c.n_orb, c.N), dtype=torch.float64, device="cuda")
+    B.bltc_convolve(full, c.k, f, c.n_orb, ref, True)
+    outs = [torch.full((c.n_orb, c.N), float("nan"), dtype=torch.float64, device="cuda") for _ in range(3)]
+    for r in range(3):                                   # "rank r" scatters its slice into all three buffers
+        plan = B.bltc_create_sharded(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, r, 3)
+        peers = [outs[q] for q in range(3) if q != r]
+        B.bltc_convolve_scatter(plan, c.k, f, c.n_orb, outs[r], peers, True)
+        torch.cuda.synchronize()
+        B.bltc_destroy(plan)
+    for o in outs:
+        assert torch.equal(o, ref)                       # every "rank" holds the whole result, bitwise the unsharded one
+    cref = torch.empty_like(ref)
+    B.bltc_convolve_coulomb(full, f, c.n_orb, cref, True, 0.2)
+    co = [torch.empty_like(ref) for _ in range(2)]
+    B.bltc_convolve_coulomb_scatter(full, f, c.n_orb, co[0], [co[1].data_ptr()], True, 0.2)      # raw addresses work too
+    torch.cuda.synchronize()
+    assert torch.equal(co[0], cref) and torch.equal(co[1], cref)
+    with pytest.raises(B.BltcError):
+        B.bltc_convolve_scatter(full, c.k, f, c.n_orb, outs[0], [outs[1]] * 16, True)            # at most 15 peers
+    B.bltc_destroy(full)
+
+
+@pytest.mark.gpu
+def test_gpu_sharded_plan_fused_scatter_over_symmetric_memory_world1():
+    # the symmetric-memory plumbing of ShardedPlan(fused_scatter=True); a 1-rank group is all one GPU allows
+    import torch
+    import torch.distributed as dist
+    from paper_2003_01833_b200.multi_gpu import ShardedPlan
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(_free_port())
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        c = I.random_cloud(6000, n_orb=3, seed=24, clustered=True, leaf_size=200, batch_size=200, degree=4)
+        X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+        f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+        try:
+            sp = ShardedPlan(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, fused_scatter=True)
+            got = sp.convolve(c.k, f, c.n_orb)
+            got2 = sp.convolve(c.k, f, c.n_orb, out=torch.empty((c.n_orb, c.N), dtype=torch.float64, device="cuda"))
+        except (RuntimeError, NotImplementedError) as e:         # symmetric memory not available on this box
+            pytest.skip(f"torch symmetric memory unavailable: {e}")
+        plan = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+        ref = torch.empty((c.n_orb, c.N), dtype=torch.float64, device="cuda")
+        B.bltc_convolve(plan, c.k, f, c.n_orb, ref)
+        torch.cuda.synchronize()
+        assert torch.equal(got, ref) and torch.equal(got2, ref)
+        sp.destroy(); B.bltc_destroy(plan)
+    finally:
+        dist.destroy_process_group()
