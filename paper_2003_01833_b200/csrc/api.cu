@@ -660,7 +660,7 @@ int convolve_impl(bltc_handle h, int kind, const double* k, double alpha, const 
                              h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[3], st));
         // a4: near field
-        BLTC_CUDA(launch_near(kind, ot, sub, guard, h->near_items.p, (int)hp.near_items.size(), h->near_ranges.p,
+        BLTC_CUDA(launch_near(kind, ot, sub, guard, false, h->near_items.p, (int)hp.near_items.size(), h->near_ranges.p,
                               h->src_rec.p, h->fsrc.p, h->tgt_rec, ftgt, nk, h->partial.p, hp.partial_len, st));
         if (ev) BLTC_CUDA(cudaEventRecord(ev[4], st));
         // a5: epilogue
@@ -876,7 +876,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             BLTC_CUDA(cudaEventCreate(&ea)); BLTC_CUDA(cudaEventCreate(&eb));
             BLTC_CUDA(cudaEventRecord(ea, st));
         }
-        BLTC_CUDA(launch_near(kind, ot, sub, guard, t_items.as<WorkItem>(), (int)items.size(), t_ranges.as<Range>(),
+        BLTC_CUDA(launch_near(kind, ot, sub, guard, true, t_items.as<WorkItem>(), (int)items.size(), t_ranges.as<Range>(),
                               t_src_rec.as<double4>(), t_fsrc.as<double>(), t_tgt_rec.as<double4>(),
                               t_ftgt.as<double>(), nk, t_partial.as<double>(), partial_len, st));
         if (g_direct_profiling) { BLTC_CUDA(cudaEventRecord(eb, st)); g_direct_pairs.emplace_back(ea, eb); }

@@ -400,7 +400,7 @@ __device__ __forceinline__ void near_tile(TargetRegs<R, OT>& T, const double* __
 
 // The work of one near-field CTA with R targets per thread (R = 2: groups of 64 targets; R = 1: the half-group tile
 // tiles that hold the tail of a ragged batch, WorkItem::rshift).
-template <int R, int OT, bool SUB, bool GUARD, int KIND>
+template <int R, int OT, bool SUB, bool GUARD, int KIND, bool ALLZS>
 __device__ __forceinline__ void near_body(const WorkItem& it, const Range* __restrict__ ranges,
                                           const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
                                           const double4* __restrict__ tgt_rec, const double* __restrict__ ftgt,
@@ -436,13 +436,17 @@ __device__ __forceinline__ void near_body(const WorkItem& it, const Range* __res
         }
         __syncthreads();
         const int j0 = (fill * split) / S, j1 = (fill * (split + 1)) / S;
-        if (flags & kRangeMayCoincide) near_tile<R, OT, SUB, GUARD, true, KIND>(T, s_tile, j0, j1, kp, tab, mr);
+        // ALLZS (direct_convolve: a target sample meets every source segment): ONE pair loop in the kernel.  With two
+        // loops ptxas keeps the exp constants of the first one in vector registers instead of uniform registers, and a
+        // DFMA with three distinct vector-register sources holds the FP64 pipe for 3 cycles instead of 2;
+        // the treecode's near field rarely needs the zero-safe loop, so it is the one that comes first.
+        if (ALLZS || (flags & kRangeMayCoincide)) near_tile<R, OT, SUB, GUARD, true, KIND>(T, s_tile, j0, j1, kp, tab, mr);
         else near_tile<R, OT, SUB, GUARD, false, KIND>(T, s_tile, j0, j1, kp, tab, mr);
     }
     reduce_and_store<R, OT>(T, it, warp, lane, split, S, s_tile, partial, partial_len);
 }
 
-template <int R, int OT, bool SUB, bool GUARD, int KIND>
+template <int R, int OT, bool SUB, bool GUARD, int KIND, bool ALLZS>
 __global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
 near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges,
             const double4* __restrict__ src_rec, const double* __restrict__ fsrc,
@@ -454,11 +458,11 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
     const MathRegs mr = math_regs_init(kMathOpaque);
     const WorkItem it = items[blockIdx.x];
     if (it.rshift == 0) {
-        near_body<R, OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+        near_body<R, OT, SUB, GUARD, KIND, ALLZS>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
     } else if (R >= 4 && it.rshift == 2) {
-        near_body<(R >= 4 ? R / 4 : 1), OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+        near_body<(R >= 4 ? R / 4 : 1), OT, SUB, GUARD, KIND, ALLZS>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
     } else {
-        near_body<(R >= 2 ? R / 2 : 1), OT, SUB, GUARD, KIND>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
+        near_body<(R >= 2 ? R / 2 : 1), OT, SUB, GUARD, KIND, ALLZS>(it, ranges, src_rec, fsrc, tgt_rec, ftgt, kp, partial, partial_len, s_tile, tab, mr);
     }
 }
 
@@ -802,11 +806,13 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
 
 template <int R, int OT, bool SUB, bool GUARD> struct FarK { static auto get() { return far_kernel<R, OT, SUB, GUARD, kYukawa, 0>; } };
 template <int R, int OT, bool SUB, bool GUARD> struct FarK9 { static auto get() { return far_kernel<R, OT, SUB, GUARD, kYukawa, 9>; } };
-template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD, kYukawa>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearK { static auto get() { return near_kernel<R, OT, SUB, GUARD, kYukawa, false>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearKZ { static auto get() { return near_kernel<R, OT, SUB, GUARD, kYukawa, true>; } };
 // Coulomb: the Gaussian's exponent -r^2/alpha^2 is not bounded by a per-launch test, so the underflow guard is always on
 template <int R, int OT, bool SUB, bool GUARD> struct FarKC { static auto get() { return far_kernel<R, OT, SUB, true, kCoulomb, 0>; } };
 template <int R, int OT, bool SUB, bool GUARD> struct FarK9C { static auto get() { return far_kernel<R, OT, SUB, true, kCoulomb, 9>; } };
-template <int R, int OT, bool SUB, bool GUARD> struct NearKC { static auto get() { return near_kernel<R, OT, SUB, true, kCoulomb>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearKC { static auto get() { return near_kernel<R, OT, SUB, true, kCoulomb, false>; } };
+template <int R, int OT, bool SUB, bool GUARD> struct NearKCZ { static auto get() { return near_kernel<R, OT, SUB, true, kCoulomb, true>; } };
 
 cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const int32_t* far_slots,
                        const double* slot_nodes, const double* what, const double* fhat, int degree,
@@ -827,16 +833,16 @@ cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkIt
                                what, fhat, degree + 1, tgt_rec, ftgt, kp, partial, partial_len);
 }
 
-cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
-                        const double4* src_rec, const double* fsrc, const double4* tgt_rec,
+cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, bool all_zero_safe, const WorkItem* items, int nitems,
+                        const Range* ranges, const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st) {
     if (nitems == 0) return cudaSuccess;
-    if (kind == kCoulomb)
-        return dispatch_pair<NearKC>(ot, subtract, true, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc,
-                                     tgt_rec, ftgt, kp, partial, partial_len);
-    return dispatch_pair<NearK>(ot, subtract, guard, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc,
-                                tgt_rec, ftgt, kp, partial, partial_len);
+#define BLTC_NEAR(K, G) dispatch_pair<K>(ot, subtract, G, near_smem_bytes(ot), nitems, st, items, ranges, src_rec, fsrc, \
+                                         tgt_rec, ftgt, kp, partial, partial_len)
+    if (kind == kCoulomb) return all_zero_safe ? BLTC_NEAR(NearKCZ, true) : BLTC_NEAR(NearKC, true);
+    return all_zero_safe ? BLTC_NEAR(NearKZ, guard) : BLTC_NEAR(NearK, guard);
+#undef BLTC_NEAR
 }
 
 cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_begin, const int32_t* b_count,

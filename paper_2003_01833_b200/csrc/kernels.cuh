@@ -61,9 +61,10 @@ cudaError_t launch_far(int kind, int ot, bool subtract, bool guard, const WorkIt
                        const double4* tgt_rec, const double* ftgt, const KPar& kp, double* partial,
                        int64_t partial_len, cudaStream_t st);
 
-// a4 / a6: near field and brute-force direct sum (same kernel, different work items)
-cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, const WorkItem* items, int nitems, const Range* ranges,
-                        const double4* src_rec, const double* fsrc, const double4* tgt_rec,
+// a4 / a6: near field and brute-force direct sum (same kernel, different work items).  all_zero_safe: every tile runs
+// the loop that skips r == 0 (direct_convolve), instead of only the ranges flagged kRangeMayCoincide
+cudaError_t launch_near(int kind, int ot, bool subtract, bool guard, bool all_zero_safe, const WorkItem* items, int nitems,
+                        const Range* ranges, const double4* src_rec, const double* fsrc, const double4* tgt_rec,
                         const double* ftgt, const KPar& kp, double* partial, int64_t partial_len,
                         cudaStream_t st);
 
