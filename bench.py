@@ -44,16 +44,22 @@ UNIT = "interactions/s"
 # FP64 instruction mix of one kernel evaluation, counted in the SASS of the inner loops
 # (profiles/r01*_sass_counts.md; tests/test_library_host.py re-counts them from the built library).  flops = 2*DFMA + DMUL + DADD.
 # key: (kernel, orbital tile width OT) -> flops per (target, source/proxy point) pair for ALL OT orbitals
-FLOPS_PER_PAIR = {
-    ("near", 1): 32.0, ("near", 2): 46.0, ("near", 3): 60.0, ("near", 4): 74.0,
-    ("far", 1): 27.0, ("far", 2): 42.0, ("far", 3): 57.0, ("far", 4): 72.0,
+def _mix(first, per_extra, div=1.0):
+    return {ot: (first + per_extra * (ot - 1)) / div for ot in range(1, 8)}
+
+
+FLOPS_PER_PAIR = {(kern, ot): v for kern, tab in {
+    "near": _mix(32.0, 14.0), "far": _mix(27.0, 15.0),
     # degree 8: far_kernel<..., N1 = 9>, one (k1, k2) row of 9 proxy points per loop trip incl. its dx^2 + dy^2
-    ("far9", 1): 239.0 / 9, ("far9", 2): 374.0 / 9, ("far9", 3): 509.0 / 9, ("far9", 4): 644.0 / 9,
+    "far9": _mix(239.0, 135.0, 9.0),
     # Coulomb kernel with Gaussian singularity subtraction (bltc_convolve_coulomb)
-    ("cnear", 1): 31.0, ("cnear", 2): 35.0, ("cnear", 3): 39.0, ("cnear", 4): 43.0,
-    ("cfar", 1): 26.0, ("cfar", 2): 30.0, ("cfar", 3): 34.0, ("cfar", 4): 38.0,
-    ("cfar9", 1): 230.0 / 9, ("cfar9", 2): 266.0 / 9, ("cfar9", 3): 302.0 / 9, ("cfar9", 4): 338.0 / 9,
-}
+    "cnear": _mix(31.0, 4.0), "cfar": _mix(26.0, 4.0), "cfar9": _mix(230.0, 36.0, 9.0),
+}.items() for ot, v in tab.items()}
+# tiles of 6-7 orbitals unroll 3 proxy points per trip instead of a whole row (kernels.cu): the inner loop executes the
+# generic far kernel's mix; the row prologue (dx^2 + dy^2, 5 flops per target and row of 9) is then NOT counted
+for _ot in (6, 7):
+    FLOPS_PER_PAIR[("far9", _ot)] = FLOPS_PER_PAIR[("far", _ot)]
+    FLOPS_PER_PAIR[("cfar9", _ot)] = FLOPS_PER_PAIR[("cfar", _ot)]
 # 148 SMs x 64 FP64 FMA lanes x 2 flops x 1.965 GHz (MEASURED_PEAKS.json sm_max_mhz); the DFMA-only
 # probe (bltc_probe_fp64) measures 36.8 TFLOP/s on this pool's B200s.
 FP64_PEAK_TFLOPS_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
@@ -67,12 +73,10 @@ def measured_hbm_gbs():
         return 6650.0
 
 
-def orbital_groups(n_orb, max_ot=4):
-    ng = (n_orb + max_ot - 1) // max_ot
-    g = [n_orb // ng] * ng
-    for i in range(n_orb % ng):
-        g[i] += 1
-    return g
+def orbital_groups(n_orb):
+    """The register tiles (orbital groups) the library cuts n_orb orbitals into: asked of the library itself."""
+    from paper_2003_01833_b200 import binding as B
+    return B.bltc_orbital_tiles(n_orb)
 
 
 class ClockSampler:

@@ -304,6 +304,15 @@ int bltc_direct_get_kernel_ms(float* ms);
  */
 int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream);
 
+/*
+ * bltc_orbital_tiles: how a call with n_orb orbitals is cut into register tiles.  The pair kernels evaluate the
+ * geometry, rsqrt and r of a (target, source) pair once for all orbitals of a tile (at most 7); the library cuts
+ * n_orb into equal-as-possible tiles whose widths minimise a measured per-orbital cost, and runs
+ * steps a1-a5 once per tile.  widths: HOST int[capacity]; returns the number of tiles (> capacity: nothing is
+ * written past capacity), or BLTC_EINVAL.  Measurement code needs it to count the executed flops of a launch.
+ */
+int bltc_orbital_tiles(int n_orb, int* widths, int capacity);
+
 const char* bltc_last_error(void);
 const char* bltc_version(void);
 

@@ -48,7 +48,7 @@ EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc
             "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
-            "bltc_probe_fp64", "bltc_last_error", "bltc_version")
+            "bltc_probe_fp64", "bltc_orbital_tiles", "bltc_last_error", "bltc_version")
 
 _lib = None
 
@@ -87,6 +87,7 @@ def lib():
     L.bltc_direct_set_profiling.argtypes = [C.c_int]
     L.bltc_direct_get_kernel_ms.argtypes = [C.POINTER(C.c_float)]
     L.bltc_probe_fp64.argtypes = [C.c_int, _dp, vp]
+    L.bltc_orbital_tiles.argtypes = [C.c_int, C.POINTER(C.c_int), C.c_int]
     for name in EXPORTED:
         f = getattr(L, name)
         if name not in ("bltc_last_error", "bltc_version"):
@@ -360,6 +361,16 @@ def bltc_probe_fp64(iters=64, stream=None):
     t = C.c_double(0)
     _check(lib().bltc_probe_fp64(int(iters), C.byref(t), _stream_ptr(stream)))
     return float(t.value)
+
+
+def bltc_orbital_tiles(n_orb):
+    """Widths of the register tiles a call with n_orb orbitals is cut into (include/bltc.h)."""
+    n = lib().bltc_orbital_tiles(int(n_orb), None, 0)
+    if n < 0:
+        _check(n)
+    w = (C.c_int * n)()
+    _check(min(0, lib().bltc_orbital_tiles(int(n_orb), w, n)))
+    return [int(v) for v in w]
 
 
 def bltc_version():

@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -122,11 +123,31 @@ cudaError_t stage_in(const double* src, size_t count, TempBuf& tmp, cudaStream_t
     return e;
 }
 
+// Orbitals are processed in groups ("tiles") of <= kMaxOT = the register tile of the pair kernels, sizes as equal as
+// possible.  The number of tiles minimises a per-orbital cost measured on B200 (near + far kernel time per orbital and
+// pair at tile width w, relative units): wider tiles share the geometry / rsqrt of a pair among more
+// orbitals (7 is what fits in 128 registers with two targets per thread).  BLTC_ORBITAL_TILE = 1 .. kMaxOT forces a maximum width
+// (tuning runs).
 std::vector<int> orbital_groups(int n_orb) {
-    const int ng = (n_orb + kMaxOT - 1) / kMaxOT;
-    std::vector<int> g(ng, n_orb / ng);
-    for (int i = 0; i < n_orb % ng; ++i) ++g[i];
-    return g;
+    static const double kCost[kMaxOT + 1] = {0.0, 116.8, 84.1, 75.0, 70.0, 67.7, 68.2, 65.7};
+    auto split = [n_orb](int ng) {
+        std::vector<int> g(ng, n_orb / ng);
+        for (int i = 0; i < n_orb % ng; ++i) ++g[i];
+        return g;
+    };
+    if (const char* e = std::getenv("BLTC_ORBITAL_TILE")) {
+        const int v = std::atoi(e);
+        if (v >= 1 && v <= kMaxOT) return split((n_orb + v - 1) / v);
+    }
+    int best_ng = (n_orb + kMaxOT - 1) / kMaxOT;
+    double best = 1e300;
+    for (int ng = best_ng; ng <= n_orb; ++ng) {
+        double c = 0.0;
+        for (int w : split(ng)) c += kCost[w] * w;
+        if (c < best) { best = c; best_ng = ng; }
+        if (n_orb / ng < 3) break;                 // narrower tiles only cost more
+    }
+    return split(best_ng);
 }
 
 // direct_convolve has no handle to carry its profiling switch and events: they are per calling thread
@@ -226,7 +247,14 @@ std::vector<int32_t> to_i32(const std::vector<int64_t>& v) {
 extern "C" {
 
 const char* bltc_last_error(void) { return g_err.c_str(); }
-const char* bltc_version(void) { return "bltc-b200 0.1 (sm_100a)"; }
+const char* bltc_version(void) { return "bltc-b200 0.2 (sm_100a)"; }
+
+int bltc_orbital_tiles(int n_orb, int* widths, int capacity) {
+    if (n_orb < 1 || (capacity > 0 && !widths)) return fail(BLTC_EINVAL, "bltc_orbital_tiles: n_orb >= 1 and a widths array are required");
+    const std::vector<int> g = orbital_groups(n_orb);
+    for (int i = 0; i < (int)g.size() && i < capacity; ++i) widths[i] = g[i];
+    return (int)g.size();
+}
 
 int bltc_create_host_plan_sharded(bltc_handle* h, const double* targets, const double* sources,
                                   const double* weights, int64_t N, double theta, int interp_degree,

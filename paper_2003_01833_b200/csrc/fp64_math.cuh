@@ -105,10 +105,13 @@ __device__ __forceinline__ double exp_neg_kr(double r, double c, uint32_t tab, c
     const double rho = fma(r, c, -nf);
     int m = __double2loint(t);
     if (GUARD) m = (__double2hiint(t) == 0x43380000) ? m : 0;
-    uint32_t r3, off, lo, hi;
-    asm("shf.l.wrap.b32 %0, %1, %1, 3;" : "=r"(r3) : "r"(m));
-    asm("and.b32 %0, %1, %2;" : "=r"(off) : "r"(r3), "n"((BLTC_EXP_T - 1) * 8));                    // 8 j
-    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(off + tab));
+    // table address = tab + 8 j: the mask first, then shift and add -- ptxas fuses the last two into one LEA on the
+    // ALU pipe whether `tab` sits in a uniform or (wide orbital tiles) a vector register; masking the shifted index
+    // instead leaves an IMAD.IADD on the FMA pipe in the second case
+    uint32_t j, j8, lo, hi;
+    asm("and.b32 %0, %1, %2;" : "=r"(j) : "r"(m), "n"(BLTC_EXP_T - 1));
+    asm("shf.l.wrap.b32 %0, %1, %2, 3;" : "=r"(j8) : "r"(0), "r"(j));
+    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(j8 + tab));
     // exponent n + 1023 merged by a shift and an add, both pinned to the ALU pipe: written as
     // hi + (m << s), ptxas emits one IMAD (m * 2^s + hi) on the FMA pipe, which steals FP64-pipe issue cycles
     uint32_t msh;

@@ -342,7 +342,7 @@ __device__ __forceinline__ void reduce_and_store(TargetRegs<R, OT>& T, const Wor
 // Shared-memory tile of sources: one record {x, y, z, w, f[OT]} per source, padded to a multiple of
 // 16 bytes, so one source is 3-4 LDS.128 at immediate offsets from one running pointer.  The S
 // source-split ways of a tile take contiguous chunks of it (broadcast reads: no bank conflicts).
-template <int OT> struct SrcRec { static constexpr int kDoubles = OT <= 2 ? 6 : 8; };
+template <int OT> struct SrcRec { static constexpr int kDoubles = 4 + 2 * ((OT + 1) / 2); };
 
 // ZS (zero-safe): the tile may hold a source that coincides with a target -> the singular term is
 // skipped by an integer select on the rsqrt seed (reading R3).  The host flags the
@@ -471,7 +471,11 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 // k3 fastest, so a (k1, k2) row of the tensor grid is n1 consecutive records.  N1 > 0: the grid size
 // degree + 1 is a compile-time constant and the k3 loop is fully unrolled (no remainder iteration, the
 // next row's dx^2 + dy^2 overlaps the tail of the current one); N1 = 0: any degree.
-template <int OT> struct ProxyRec { static constexpr int kDoubles = OT == 1 ? 2 : (OT <= 3 ? 4 : 6); };
+template <int OT> struct ProxyRec {
+    static constexpr int kDoubles = 2 * ((OT + 2) / 2);
+    // tile of proxy points: 64 KB (exp table) + tile must fit twice in an SM's 227 KB of shared memory
+    static constexpr int kTile = OT <= 4 ? kProxyTile : 768;
+};
 
 // KIND = kCoulomb: acc += (fhat_k - f_i what_k e^{-r^2/alpha^2}) / r  (reading R21: the Gaussian of Eq. (23)
 // is interpolated with the proxy weights of w).
@@ -483,11 +487,14 @@ __device__ __forceinline__ void far_body(const WorkItem& it, const int32_t* __re
                                          const KPar& kp, double* __restrict__ partial, int64_t partial_len,
                                          double* s_pts, uint32_t tab, const MathRegs& mr) {
     constexpr int PD = ProxyRec<OT>::kDoubles;
-    static_assert(kProxyTile * PD >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
-    constexpr int kU = N1 ? N1 : kFarUnroll;
+    constexpr int PT = ProxyRec<OT>::kTile;
+    static_assert(PT * PD >= R * OT * kPairWarps * 32, "reduction scratch fits in the tile");
+    // compile-time grid size: the k3 loop is fully unrolled up to 5 orbitals; wider tiles unroll 3 proxy points per
+    // trip (fully unrolled they spill registers: far kernel at 7 orbitals 567 -> 520 ms on the cfg1 mesh x 21 orbitals)
+    constexpr int kU = N1 ? (OT >= 6 ? 3 : N1) : kFarUnroll;
     const int n1 = N1 ? N1 : n1_arg;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double* s_nodes = s_pts + kProxyTile * PD;           // [3][21]
+    double* s_nodes = s_pts + PT * PD;                   // [3][21]
     const ExpConst ec{kp.c1, kp.c3};
     const int G = 1 << it.gshift, S = kPairWarps >> it.gshift;
     const int grp = warp & (G - 1), split = warp >> it.gshift;
@@ -496,7 +503,7 @@ __device__ __forceinline__ void far_body(const WorkItem& it, const int32_t* __re
 
     const int plane = n1 * n1;
     const int P = plane * n1;
-    const int planes_per_chunk = max(1, kProxyTile / plane);
+    const int planes_per_chunk = max(1, PT / plane);
     for (int q = it.list_begin; q < it.list_end; ++q) {
         const int slot = far_slots[q];
         for (int k1a = 0; k1a < n1; k1a += planes_per_chunk) {
@@ -643,8 +650,10 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
-size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + (size_t)kSrcTile * sizeof(double) * (ot <= 2 ? 6 : 8); }
-size_t far_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)kProxyTile * (ot == 1 ? 2 : (ot <= 3 ? 4 : 6)) + 3 * 21); }
+size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + (size_t)kSrcTile * sizeof(double) * (4 + 2 * ((ot + 1) / 2)); }
+size_t far_smem_bytes(int ot) {
+    return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)(ot <= 4 ? kProxyTile : 768) * (2 * ((ot + 2) / 2)) + 3 * 21);
+}
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {
@@ -746,7 +755,7 @@ cudaError_t launch_upward(int ot, const UpItem* items, int nitems, const UpReduc
         }                                                                                              \
         break;
     switch (ot) {
-        BLTC_UP(0) BLTC_UP(1) BLTC_UP(2) BLTC_UP(3) BLTC_UP(4)
+        BLTC_UP(0) BLTC_UP(1) BLTC_UP(2) BLTC_UP(3) BLTC_UP(4) BLTC_UP(5) BLTC_UP(6) BLTC_UP(7)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_UP
@@ -773,6 +782,9 @@ cudaError_t launch_upward_children(int ot, const C2PItem* items, int nitems, con
         case 2: BLTC_C2P(2)
         case 3: BLTC_C2P(3)
         case 4: BLTC_C2P(4)
+        case 5: BLTC_C2P(5)
+        case 6: BLTC_C2P(6)
+        case 7: BLTC_C2P(7)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_C2P
@@ -798,6 +810,9 @@ cudaError_t dispatch_pair(int ot, bool subtract, bool guard, size_t smem, int gr
         case 2: BLTC_SG(kTargetsPerThread, 2)
         case 3: BLTC_SG(kTargetsPerThread, 3)
         case 4: BLTC_SG(kTargetsPerThread, 4)
+        case 5: BLTC_SG(kTargetsPerThread, 5)
+        case 6: BLTC_SG(kTargetsPerThread, 6)
+        case 7: BLTC_SG(kTargetsPerThread, 7)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_SG
@@ -858,7 +873,7 @@ cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_
             b_partial_base, b_nseg, partial, partial_len, ftgt, kp, perm, out, stride, o0);            \
         break;
     switch (ot) {
-        BLTC_EPI(1) BLTC_EPI(2) BLTC_EPI(3) BLTC_EPI(4)
+        BLTC_EPI(1) BLTC_EPI(2) BLTC_EPI(3) BLTC_EPI(4) BLTC_EPI(5) BLTC_EPI(6) BLTC_EPI(7)
         default: return cudaErrorInvalidValue;
     }
 #undef BLTC_EPI

@@ -7,11 +7,11 @@
 
 namespace bltc {
 
-constexpr int kMaxOT = 4;          // orbitals processed together in one pass (register tile)
+constexpr int kMaxOT = 7;          // orbitals processed together in one pass (register tile; 7 measured best)
 constexpr int kThreads = 256;      // 8 warps per CTA (upward pass, epilogue, utilities)
 constexpr int kPairThreads = 32 * kPairWarps;   // pair kernels (plan_host.hpp)
 constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (near field / direct)
-constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field)
+constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field), OT <= 4; 768 above (kernels.cu)
 
 // kTargetsPerThread (plan_host.hpp): targets per thread of a full tile, R = 2 for every orbital-tile width -- one staged
 // source / proxy record feeds two pair evaluations (measured on B200: near -8 %, far -2 % at OT = 4 against R = 1)
