@@ -251,7 +251,26 @@ def run_reference(args):
     return 0
 
 
-def roofline_of(phase_ms, st, groups, degree, coulomb, probe, steps):
+# FP64 instructions per (target, source / proxy point) pair of a tile of ot orbitals, as (first orbital, each further one),
+# counted in the SASS (python -m paper_2003_01833_b200.sass_count), and how many of them are DFMAs with three distinct
+# vector-register sources -- those hold the FP64 pipe for 3 cycles instead of 2 on sm_100a (profiles/r02h_probes.md)
+FP64_INSTR_PER_PAIR = {"near": (22.0, 9.0), "far": (17.0, 9.0), "far9": (148.0 / 9, 9.0)}
+FP64_3REG_PER_PAIR = {"near": 1.0, "far": 2.0, "far9": 2.0}            # per orbital: the accumulate (+ fhat - f_i what)
+
+
+def fp64_pipe_busy(key, groups, evals, ms, sm_mhz, n_sm=148):
+    """Share of the FP64 pipe's cycles that the kernel's FP64 instructions occupy: (2 cycles per instruction + 1 per
+    three-register DFMA) x warp instructions / (4 sub-partitions x SMs x clock x time).  None for the Coulomb kernels."""
+    if key not in FP64_INSTR_PER_PAIR or not sm_mhz or ms <= 0:
+        return None
+    cyc = 0.0
+    for g in groups:
+        first, extra = FP64_INSTR_PER_PAIR["far" if key == "far9" and g >= 6 else key]   # 6-7 orbitals: 3 points per trip
+        cyc += evals / 32.0 * (2.0 * (first + extra * (g - 1)) + FP64_3REG_PER_PAIR[key] * g)
+    return cyc / (4.0 * n_sm * sm_mhz * 1e6 * ms * 1e-3)
+
+
+def roofline_of(phase_ms, st, groups, degree, coulomb, probe, steps, sm_mhz=None):
     """FP64-ALU roofline of the two pair kernels from the library's per-phase CUDA events: executed FP64 flops
     (SASS-counted mix x the plan's exact pair counts, summed over the orbital groups of one step) / kernel time."""
     pre = "c" if coulomb else ""
@@ -267,7 +286,8 @@ def roofline_of(phase_ms, st, groups, degree, coulomb, probe, steps):
                      "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md 6)",
                      "peak_measured_dfma_probe": probe, "launches_per_step": len(groups),
                      "orbital_tiles": groups, "avg_launch_ms": ms / len(groups),
-                     "flops_per_launch": flops / len(groups), "ms_per_step": ms}
+                     "flops_per_launch": flops / len(groups), "ms_per_step": ms,
+                     "fp64_pipe_busy": fp64_pipe_busy(key, groups, evals, ms, sm_mhz)}
     return out
 
 
@@ -342,6 +362,13 @@ def run_cuda(args):
         else:
             plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
         create_ms = (time.perf_counter() - t0) * 1e3
+        create_cold_ms = create_ms
+        if not shard:                                    # the first build pays module load and pool growth: time a second
+            B.bltc_destroy(plan)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
+            create_ms = (time.perf_counter() - t0) * 1e3
         st = B.bltc_get_stats(plan)
 
         def convolve(f_, out_):
@@ -422,7 +449,7 @@ def run_cuda(args):
             same = bool(torch.equal(res.cpu(), out.cpu()))
             e2e = {"ms_per_step": e2e_ms, "steps": e2e_steps, "bitwise_equal_to_device_path": same}
         return dict(plan=plan, st=st, X=X, w=w, f=f, out=out, ms_per_step=ms_per_step, phase_sum=phase_sum,
-                    create_ms=create_ms, clocks=clocks, e2e=e2e)
+                    create_ms=create_ms, create_cold_ms=create_cold_ms, clocks=clocks, e2e=e2e)
 
     # ---- the headline workload ----------------------------------------------------------------
     c = workload(args.workload, args.kernel, args.orbitals)
@@ -493,10 +520,12 @@ def run_cuda(args):
               "note": "L2 flushed before each call; 4 dependent streaming kernels"}
         del phi, psi_old
     probe = B.bltc_probe_fp64(64) if rank == 0 else None
+    probe3 = B.bltc_probe_fp64(64, form=1) if rank == 0 else None      # three-register DFMAs: 2/3 of the pipe's peak
     stq = dict(st, near_evals=st["shard_near_evals"], far_evals=st["shard_far_evals"]) if sharded else st
-    roof = roofline_of(R["phase_sum"], stq, groups, c.degree, coulomb, probe, args.steps) if rank == 0 else None
+    roof = (roofline_of(R["phase_sum"], stq, groups, c.degree, coulomb, probe, args.steps, R["clocks"].get("sm_mhz"))
+            if rank == 0 else None)
     phase_ms = {p: v / args.steps for p, v in R["phase_sum"].items()}
-    create_ms, clocks, e2e_info = R["create_ms"], R["clocks"], R["e2e"]
+    create_ms, create_cold_ms, clocks, e2e_info = R["create_ms"], R["create_cold_ms"], R["clocks"], R["e2e"]
     B.bltc_destroy(plan)
     del X, w, f, out, R
 
@@ -505,7 +534,8 @@ def run_cuda(args):
     if rank == 0 and world == 1 and args.workload == "cfg3" and not coulomb and not args.orbitals:
         c1 = workload("cfg1", args.kernel, 0)
         R1 = time_workload(c1, 5, 3, False, 0, False)
-        r1 = roofline_of(R1["phase_sum"], R1["st"], orbital_groups(c1.n_orb), c1.degree, False, probe, 5)
+        r1 = roofline_of(R1["phase_sum"], R1["st"], orbital_groups(c1.n_orb), c1.degree, False, probe, 5,
+                         clocks.get("sm_mhz"))
         cfg1 = {"workload": c1.name, "N": c1.N, "n_orb": c1.n_orb, "ms_per_step": R1["ms_per_step"],
                 "value": c1.n_orb * float(c1.N) ** 2 / (R1["ms_per_step"] * 1e-3), "steps": 5,
                 "near_frac": r1["near"]["frac"], "far_frac": r1["far"]["frac"],
@@ -527,10 +557,14 @@ def run_cuda(args):
             "time_per_convolution_ms": ms_per_step / O,
             "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * jobs / (ms_per_step * 1e-3),
             "phase_ms": phase_ms,
-            "plan": {"create_ms": create_ms, "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
+            "plan": {"create_ms": create_ms, "create_cold_ms": create_cold_ms,
+                     "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
                      "clusters": st["n_clusters"], "batches": st["n_batches"],
                      "far_evals": st["far_evals"], "near_evals": st["near_evals"]},
             "roofline": roof[dom], "roofline_" + other: roof[other],
+            "dfma_probe_tflops": {"two_register_sources": probe, "three_register_sources": probe3,
+                                  "note": "DFMA-only kernels (bltc_probe_fp64_form): a DFMA with three distinct vector-"
+                                          "register sources holds the FP64 pipe for 3 cycles instead of 2"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": O * N * 8,
                     "d2h_bytes_per_step": O * N * 8, "ms_per_step": e2e_info["ms_per_step"],
                     "steps": e2e_info["steps"],

@@ -48,7 +48,7 @@ EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc
             "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
-            "bltc_probe_fp64", "bltc_orbital_tiles", "bltc_last_error", "bltc_version")
+            "bltc_probe_fp64", "bltc_probe_fp64_form", "bltc_orbital_tiles", "bltc_last_error", "bltc_version")
 
 _lib = None
 
@@ -87,6 +87,7 @@ def lib():
     L.bltc_direct_set_profiling.argtypes = [C.c_int]
     L.bltc_direct_get_kernel_ms.argtypes = [C.POINTER(C.c_float)]
     L.bltc_probe_fp64.argtypes = [C.c_int, _dp, vp]
+    L.bltc_probe_fp64_form.argtypes = [C.c_int, C.c_int, _dp, vp]
     L.bltc_orbital_tiles.argtypes = [C.c_int, C.POINTER(C.c_int), C.c_int]
     for name in EXPORTED:
         f = getattr(L, name)
@@ -357,9 +358,10 @@ def bltc_direct_get_kernel_ms():
     return float(ms.value)
 
 
-def bltc_probe_fp64(iters=64, stream=None):
+def bltc_probe_fp64(iters=64, stream=None, form=0):
+    """DFMA-only probe in TFLOP/s; form 1 = three distinct vector-register sources per DFMA (include/bltc.h)."""
     t = C.c_double(0)
-    _check(lib().bltc_probe_fp64(int(iters), C.byref(t), _stream_ptr(stream)))
+    _check(lib().bltc_probe_fp64_form(int(form), int(iters), C.byref(t), _stream_ptr(stream)))
     return float(t.value)
 
 

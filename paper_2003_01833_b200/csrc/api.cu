@@ -978,12 +978,14 @@ int bltc_gi_update(const double* w, const double* psi_old, const double* f_old, 
     return BLTC_OK;
 }
 
-int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream) {
-    if (!tflops || iters < 1) return fail(BLTC_EINVAL, "bad argument");
+int bltc_probe_fp64_form(int form, int iters, double* tflops, bltc_stream stream) {
+    if (!tflops || iters < 1 || form < 0 || form > 1) return fail(BLTC_EINVAL, "bad argument");
     float ms = 0.f; double dfma = 0.0;
-    BLTC_CUDA(launch_fp64_probe(iters, &ms, &dfma, static_cast<cudaStream_t>(stream)));
+    BLTC_CUDA(launch_fp64_probe(form, iters, &ms, &dfma, static_cast<cudaStream_t>(stream)));
     *tflops = 2.0 * dfma / (ms * 1e-3) / 1e12;
     return BLTC_OK;
 }
+
+int bltc_probe_fp64(int iters, double* tflops, bltc_stream stream) { return bltc_probe_fp64_form(0, iters, tflops, stream); }
 
 }  // extern "C"

@@ -632,17 +632,25 @@ epilogue_kernel(const int32_t* __restrict__ b_begin, const int32_t* __restrict__
 }
 
 // ------------------------------------------------------------------------------------ probe
+// FORM 0: a = fma(a, m, c) with m, c the same for every chain (held in the operand-reuse cache): the FP64 pipe's peak.
+// FORM 1: a = fma(b_i, d_j, a) -- three distinct vector-register sources per instruction, nothing to reuse: such a
+//         DFMA holds the pipe for 3 cycles instead of 2 on sm_100a (the accumulate of the pair kernels is of this form).
+template <int FORM>
 __global__ void __launch_bounds__(kThreads)
 fp64_probe_kernel(int iters, double seed, double* sink) {
-    double a[8];
+    double a[8], b[8], d[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) a[i] = seed + (double)(threadIdx.x + i);
+    for (int i = 0; i < 8; ++i) {
+        a[i] = seed + (double)(threadIdx.x + i);
+        b[i] = 1.0 + 1e-9 * (double)(threadIdx.x + i);
+        d[i] = 1e-12 * (double)(3 * threadIdx.x + i);
+    }
     const double m = 1.0 + 1e-9 * seed, c = 1e-12;
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int u = 0; u < 64; ++u)
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+            for (int i = 0; i < 8; ++i) a[i] = FORM == 0 ? fma(a[i], m, c) : fma(b[i], d[i], a[i]);
     }
     double s = 0.0;
 #pragma unroll
@@ -880,7 +888,7 @@ cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_
     return cudaGetLastError();
 }
 
-cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStream_t st) {
+cudaError_t launch_fp64_probe(int form, int iters, float* ms, double* dfma_count, cudaStream_t st) {
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -892,9 +900,13 @@ cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStre
     cudaEvent_t a, b;
     cudaEventCreate(&a); cudaEventCreate(&b);
     const int grid = sms * 8;
-    fp64_probe_kernel<<<grid, kThreads, 0, st>>>(4, 1.0, sink);          // warm-up
+    auto run = [&](int n) {
+        if (form == 0) fp64_probe_kernel<0><<<grid, kThreads, 0, st>>>(n, 1.0, sink);
+        else fp64_probe_kernel<1><<<grid, kThreads, 0, st>>>(n, 1.0, sink);
+    };
+    run(4);                                                              // warm-up
     cudaEventRecord(a, st);
-    fp64_probe_kernel<<<grid, kThreads, 0, st>>>(iters, 1.0, sink);
+    run(iters);
     cudaEventRecord(b, st);
     e = cudaEventSynchronize(b);
     if (e == cudaSuccess) e = cudaEventElapsedTime(ms, a, b);

@@ -80,7 +80,8 @@ cudaError_t launch_epilogue(int ot, bool subtract, int nbatch, const int32_t* b_
                             int64_t partial_len, const double* ftgt, const EpiPar& ep, const int32_t* perm,
                             const OutSet& outs, int64_t stride, int o0, cudaStream_t st);
 
-// roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed
-cudaError_t launch_fp64_probe(int iters, float* ms, double* dfma_count, cudaStream_t st);
+// roofline probe: DFMA-only kernel; returns elapsed ms and the number of DFMAs executed.  form 0: two register sources
+// + a reused one (the pipe's peak); form 1: three distinct vector-register sources per DFMA (3 pipe cycles instead of 2)
+cudaError_t launch_fp64_probe(int form, int iters, float* ms, double* dfma_count, cudaStream_t st);
 
 }  // namespace bltc
