@@ -129,7 +129,8 @@ cudaError_t stage_in(const double* src, size_t count, TempBuf& tmp, cudaStream_t
 // orbitals (7 is what fits in 128 registers with two targets per thread).  BLTC_ORBITAL_TILE = 1 .. kMaxOT forces a maximum width
 // (tuning runs).
 std::vector<int> orbital_groups(int n_orb) {
-    static const double kCost[kMaxOT + 1] = {0.0, 116.8, 84.1, 75.0, 70.0, 67.7, 68.2, 65.7};
+    // ms per orbital of one near + one far launch on the configs[1] mesh at tile widths 1..7 (profiles/r02f, r02h)
+    static const double kCost[kMaxOT + 1] = {0.0, 116.8, 84.1, 75.0, 70.0, 68.0, 66.6, 65.6};
     auto split = [n_orb](int ng) {
         std::vector<int> g(ng, n_orb / ng);
         for (int i = 0; i < n_orb % ng; ++i) ++g[i];
