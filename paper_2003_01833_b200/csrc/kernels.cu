@@ -342,7 +342,8 @@ __device__ __forceinline__ void reduce_and_store(TargetRegs<R, OT>& T, const Wor
 // Shared-memory tile of sources: one record {x, y, z, w, f[OT]} per source, padded to a multiple of
 // 16 bytes, so one source is 3-4 LDS.128 at immediate offsets from one running pointer.  The S
 // source-split ways of a tile take contiguous chunks of it (broadcast reads: no bank conflicts).
-template <int OT> struct SrcRec { static constexpr int kDoubles = 4 + 2 * ((OT + 1) / 2); };
+constexpr int src_rec_doubles(int ot) { return 4 + 2 * ((ot + 1) / 2); }
+template <int OT> struct SrcRec { static constexpr int kDoubles = src_rec_doubles(OT); };
 
 // ZS (zero-safe): the tile may hold a source that coincides with a target -> the singular term is
 // skipped by an integer select on the rsqrt seed (reading R3).  The host flags the
@@ -471,10 +472,12 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 // k3 fastest, so a (k1, k2) row of the tensor grid is n1 consecutive records.  N1 > 0: the grid size
 // degree + 1 is a compile-time constant and the k3 loop is fully unrolled (no remainder iteration, the
 // next row's dx^2 + dy^2 overlaps the tail of the current one); N1 = 0: any degree.
+constexpr int proxy_rec_doubles(int ot) { return 2 * ((ot + 2) / 2); }
+// tile of proxy points: 64 KB (exp table) + tile must fit twice in an SM's 227 KB of shared memory
+constexpr int proxy_tile(int ot) { return ot <= 4 ? kProxyTile : 768; }
 template <int OT> struct ProxyRec {
-    static constexpr int kDoubles = 2 * ((OT + 2) / 2);
-    // tile of proxy points: 64 KB (exp table) + tile must fit twice in an SM's 227 KB of shared memory
-    static constexpr int kTile = OT <= 4 ? kProxyTile : 768;
+    static constexpr int kDoubles = proxy_rec_doubles(OT);
+    static constexpr int kTile = proxy_tile(OT);
 };
 
 // KIND = kCoulomb: acc += (fhat_k - f_i what_k e^{-r^2/alpha^2}) / r  (reading R21: the Gaussian of Eq. (23)
@@ -658,10 +661,13 @@ fp64_probe_kernel(int iters, double seed, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
-size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + (size_t)kSrcTile * sizeof(double) * (4 + 2 * ((ot + 1) / 2)); }
+size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + sizeof(double) * (size_t)kSrcTile * src_rec_doubles(ot); }
 size_t far_smem_bytes(int ot) {
-    return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)(ot <= 4 ? kProxyTile : 768) * (2 * ((ot + 2) / 2)) + 3 * 21);
+    return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)proxy_tile(ot) * proxy_rec_doubles(ot) + 3 * 21);
 }
+static_assert(2 * (kExpTableSmemBytes + 8 * kSrcTile * src_rec_doubles(kMaxOT) + 1024) <= 228 * 1024 &&
+              2 * (kExpTableSmemBytes + 8 * (proxy_tile(kMaxOT) * proxy_rec_doubles(kMaxOT) + 63) + 1024) <= 228 * 1024,
+              "two pair-kernel CTAs (+ 1 KB reserved each) fit in an SM's shared memory at the widest orbital tile");
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {
