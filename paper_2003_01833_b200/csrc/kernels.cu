@@ -473,8 +473,8 @@ near_kernel(const WorkItem* __restrict__ items, const Range* __restrict__ ranges
 // degree + 1 is a compile-time constant and the k3 loop is fully unrolled (no remainder iteration, the
 // next row's dx^2 + dy^2 overlaps the tail of the current one); N1 = 0: any degree.
 constexpr int proxy_rec_doubles(int ot) { return 2 * ((ot + 2) / 2); }
-// tile of proxy points: 64 KB (exp table) + tile must fit twice in an SM's 227 KB of shared memory
-constexpr int proxy_tile(int ot) { return ot <= 4 ? kProxyTile : 768; }
+// tile of proxy points: 64 KB (exp table) + tile must fit kPairCtasPerSm times in an SM's 227 KB of shared memory
+constexpr int proxy_tile(int ot) { return (ot <= 4 || kPairCtasPerSm == 1) ? kProxyTile : 768; }
 template <int OT> struct ProxyRec {
     static constexpr int kDoubles = proxy_rec_doubles(OT);
     static constexpr int kTile = proxy_tile(OT);
@@ -665,9 +665,9 @@ size_t near_smem_bytes(int ot) { return (size_t)kExpTableSmemBytes + sizeof(doub
 size_t far_smem_bytes(int ot) {
     return (size_t)kExpTableSmemBytes + sizeof(double) * ((size_t)proxy_tile(ot) * proxy_rec_doubles(ot) + 3 * 21);
 }
-static_assert(2 * (kExpTableSmemBytes + 8 * kSrcTile * src_rec_doubles(kMaxOT) + 1024) <= 228 * 1024 &&
-              2 * (kExpTableSmemBytes + 8 * (proxy_tile(kMaxOT) * proxy_rec_doubles(kMaxOT) + 63) + 1024) <= 228 * 1024,
-              "two pair-kernel CTAs (+ 1 KB reserved each) fit in an SM's shared memory at the widest orbital tile");
+static_assert(kPairCtasPerSm * (kExpTableSmemBytes + 8 * kSrcTile * src_rec_doubles(kMaxOT) + 1024) <= 228 * 1024 &&
+              kPairCtasPerSm * (kExpTableSmemBytes + 8 * (proxy_tile(kMaxOT) * proxy_rec_doubles(kMaxOT) + 63) + 1024) <= 228 * 1024,
+              "the resident pair-kernel CTAs (+ 1 KB reserved each) fit in an SM's shared memory at the widest orbital tile");
 
 template <typename K>
 cudaError_t set_smem(K kernel, size_t bytes) {

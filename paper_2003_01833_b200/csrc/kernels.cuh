@@ -10,7 +10,7 @@ namespace bltc {
 constexpr int kMaxOT = 7;          // orbitals processed together in one pass (register tile; 7 measured best)
 constexpr int kThreads = 256;      // 8 warps per CTA (upward pass, epilogue, utilities)
 constexpr int kPairThreads = 32 * kPairWarps;   // pair kernels (plan_host.hpp)
-constexpr int kSrcTile = 512;      // sources staged per shared-memory tile (near field / direct)
+constexpr int kSrcTile = kPairWarps > 8 ? 1024 : 512;   // sources staged per shared-memory tile (near field / direct)
 constexpr int kProxyTile = 1024;   // proxy points staged per shared-memory tile (far field), OT <= 4; 768 above (kernels.cu)
 
 // kTargetsPerThread (plan_host.hpp): targets per thread of a full tile, R = 2 for every orbital-tile width -- one staged
