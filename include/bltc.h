@@ -280,7 +280,8 @@ int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
  *   proxy_cluster[n_proxy_clusters]          cluster id of each proxy slot
  *   nodes[n_proxy_clusters][3][n+1]          Eq. (37) mapped to the cluster box
  *   what[n_proxy_clusters][(n+1)^3]          proxy weights of w
- *   fhat[n_proxy_clusters][(n+1)^3][ot]      proxy charges of f*w for the `*ot` orbitals of that group
+ *   fhat[n_proxy_clusters][(n+1)^3][ot]      proxy charges of f*w for the `*ot` orbitals of that group; the buffer
+ *                                            must hold BLTC_MAX_ORBITAL_TILE orbitals (ot is known only afterwards)
  * Synchronises the device.
  */
 int bltc_export_proxy(bltc_handle h, int32_t* proxy_cluster, double* nodes, double* what,
@@ -315,6 +316,7 @@ int bltc_probe_fp64_form(int form, int iters, double* tflops, bltc_stream stream
  * steps a1-a5 once per tile.  widths: HOST int[capacity]; returns the number of tiles (> capacity: nothing is
  * written past capacity), or BLTC_EINVAL.  Measurement code needs it to count the executed flops of a launch.
  */
+#define BLTC_MAX_ORBITAL_TILE 7
 int bltc_orbital_tiles(int n_orb, int* widths, int capacity);
 
 const char* bltc_last_error(void);

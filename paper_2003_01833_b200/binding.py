@@ -41,6 +41,8 @@ class bltc_stats(C.Structure):
         ("built_on_device", C.c_int32), ("upward_from_children", C.c_int32)]
 
 
+MAX_ORBITAL_TILE = 7          # BLTC_MAX_ORBITAL_TILE of include/bltc.h
+
 EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc_create_host_plan_sharded",
             "bltc_create_with_builder",
             "bltc_get_shard_targets", "bltc_convolve", "direct_convolve", "bltc_convolve_scatter",
@@ -330,7 +332,7 @@ def bltc_export_proxy(plan):
     ns, n1 = st["n_proxy_clusters"], st["interp_degree"] + 1
     P = n1 ** 3
     cl = np.empty(ns, np.int32); nodes = np.empty((ns, 3, n1)); what = np.empty((ns, P))
-    fhat = np.zeros((ns, P, 4)); ot = C.c_int32(0)
+    fhat = np.zeros((ns, P, MAX_ORBITAL_TILE)); ot = C.c_int32(0)      # sized for the widest tile (include/bltc.h)
     _check(lib().bltc_export_proxy(plan._h, cl.ctypes.data_as(_i32p), nodes.ctypes.data_as(_dp),
                                    what.ctypes.data_as(_dp), fhat.ctypes.data_as(_dp), C.byref(ot)))
     o = ot.value

@@ -128,6 +128,7 @@ cudaError_t stage_in(const double* src, size_t count, TempBuf& tmp, cudaStream_t
 // pair at tile width w, relative units): wider tiles share the geometry / rsqrt of a pair among more
 // orbitals (7 is what fits in 128 registers with two targets per thread).  BLTC_ORBITAL_TILE = 1 .. kMaxOT forces a maximum width
 // (tuning runs).
+static_assert(kMaxOT == BLTC_MAX_ORBITAL_TILE, "include/bltc.h states the widest orbital tile");
 std::vector<int> orbital_groups(int n_orb) {
     // ms per orbital of one near + one far launch on the configs[1] mesh at tile widths 1..7 (profiles/r02f, r02h)
     static const double kCost[kMaxOT + 1] = {0.0, 116.8, 84.1, 75.0, 70.0, 68.0, 66.6, 65.6};

@@ -113,3 +113,28 @@ def test_result_does_not_depend_on_the_tile_width(gpu, degree):
             assert np.array_equal(cout, cref) and np.array_equal(cdout, cdref), cap
     finally:
         os.environ.pop("BLTC_ORBITAL_TILE", None)
+
+
+@pytest.mark.gpu
+def test_proxy_charges_of_a_seven_orbital_tile_against_the_oracle(gpu):
+    """The upward pass of the widest tile (upward_kernel<7>, upward_children_kernel<7>): proxy charges of all 7 orbitals
+    of the exported group against the oracle's Eq. (35), <= 1e-13; bltc_export_proxy's buffer holds the widest tile."""
+    import oracle
+    torch, B = gpu
+    os.environ.pop("BLTC_ORBITAL_TILE", None)
+    c = I.random_cloud(5000, n_orb=7, seed=14, clustered=True, leaf_size=100, batch_size=100, degree=4)
+    X, w, f = dev(torch, c.coords()), dev(torch, c.w), dev(torch, c.f)
+    plan = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+    out = torch.empty((7, c.N), dtype=torch.float64, device="cuda")
+    B.bltc_convolve(plan, c.k, f, 7, out, True)
+    torch.cuda.synchronize()
+    pr = B.bltc_export_proxy(plan)
+    assert pr["fhat"].shape[2] == 7 and B.MAX_ORBITAL_TILE == 7 and len(pr["cluster"]) > 10
+    op = oracle.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    for s in range(0, len(pr["cluster"]), 5):
+        cl = pr["cluster"][s]
+        for o in range(7):
+            fref, nodes_ref = op.proxy(cl, c.f[o] * c.w)
+            np.testing.assert_array_equal(pr["nodes"][s], nodes_ref)
+            assert np.abs(pr["fhat"][s][:, o] - fref).max() <= 1e-13 * max(np.abs(fref).max(), 1e-300), (s, o)
+    B.bltc_destroy(plan)
