@@ -13,10 +13,12 @@
 // through shared memory in a fixed order and written to a per-(batch, segment) slice of the
 // partial buffer; the epilogue adds the slices in a fixed order => bitwise reproducible results.
 //
-// The bound is the FP64 pipe: per (target, source) pair and orbital tile of OT = 1 / 2 / 3 / 4
-// orbitals the near kernel executes 22 / 31 / 40 / 49 FP64 instructions and the far kernel (n = 8) 16.4 / 25.4 /
-// 34.4 / 43.4; everything else (LDS, MUFU seed, integer exponent work, loop control) issues in the shadow of the
-// half-rate FP64 pipe, except that at OT >= 3 the exp-table lookups bring the shared-memory pipe to the same load.
+// The bound is the FP64 pipe: per (target, source) pair and orbital tile of OT = 1 ... 7 orbitals the near
+// kernel executes 22 + 9 (OT - 1) FP64 instructions and the far kernel (n = 8) 16.4 + 9 (OT - 1) -- the geometry, rsqrt and r
+// of a pair are shared by the tile; everything else (LDS, MUFU seed, integer exponent work, loop control) issues in the
+// shadow of the half-rate FP64 pipe at ~0.75 cycles per instruction, and from OT = 4 on the exp-table gathers bring the
+// shared-memory pipe to the same load (96 % at OT = 7).  A DFMA with three distinct vector-register sources holds the pipe
+// for 3 cycles instead of 2: constants are kept in uniform registers / immediates wherever ptxas allows.
 #include "kernels.cuh"
 
 #include "fp64_math.cuh"
