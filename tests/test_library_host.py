@@ -112,7 +112,13 @@ def test_bench_flops_table_matches_the_built_sass():
         assert bench.FLOPS_PER_PAIR[key] == pytest.approx(r["flops"], abs=1e-9), (key, r)
         assert r["R"] == 2
         seen.add(key)
+        if name in bench.FP64_INSTR_PER_PAIR:       # the instruction counts behind bench.py's fp64_pipe_busy
+            first, extra = bench.FP64_INSTR_PER_PAIR["far" if name == "far9" and r["OT"] >= 6 else name]
+            assert r["fp64"] == pytest.approx(first + extra * (r["OT"] - 1), abs=1e-9), (key, r)
     assert seen == set(bench.FLOPS_PER_PAIR)
+    # one pipe: 76 FP64 instructions + 7 three-register accumulates per pair of a 7-orbital near tile
+    busy = bench.fp64_pipe_busy("near", [7], 32.0 * 4 * 148 * 1.0e6, 1e3, 1.0)     # 1 s at 1 MHz: 4 x 148 x 1e6 pipe cycles
+    assert busy == pytest.approx(2 * 76 + 7)
 
 
 def test_host_plan_fuzz_against_oracle_tree(oracle_mod):
