@@ -138,3 +138,21 @@ def test_proxy_charges_of_a_seven_orbital_tile_against_the_oracle(gpu):
             np.testing.assert_array_equal(pr["nodes"][s], nodes_ref)
             assert np.abs(pr["fhat"][s][:, o] - fref).max() <= 1e-13 * max(np.abs(fref).max(), 1e-300), (s, o)
     B.bltc_destroy(plan)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n_orb", [5, 7])
+def test_underflow_guard_variants_of_the_wide_tiles(gpu, n_orb):
+    """k r up to ~7000 >> 708: the launch takes the GUARD = true instantiations (exp below 2^-1022 is replaced by a
+    subnormal-sized value, fp64_math.cuh); most pairs underflow, the nearest neighbours carry the result."""
+    import oracle
+    c = I.random_cloud(2049, n_orb=n_orb, seed=5 + n_orb, clustered=True, leaf_size=150, batch_size=150, degree=8)
+    c.k = c.k * 800.0
+    P = (c.x, c.y, c.z)
+    sample = np.arange(0, c.N, 3)
+    out, dout = run_gpu(gpu, c, sample=sample)
+    assert np.all(np.isfinite(out)) and np.all(np.isfinite(dout))
+    op = oracle.OraclePlan(P, c.theta, c.degree, c.leaf_size, c.batch_size)
+    assert rel2(out, op.evaluate(c.w, c.f, c.k)) <= TOL_BLTC
+    Ps = tuple(a[sample] for a in P)
+    assert rel2(dout, oracle.direct(Ps, P, c.w, c.f, c.k, f_tgt=c.f[:, sample])) <= TOL_DIRECT
