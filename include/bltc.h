@@ -254,6 +254,42 @@ int bltc_gi_update(const double* w, const double* psi_old, const double* f_old, 
                    const double* phi, int n_prev, int64_t N, double eps_old, double* result,
                    bltc_stream stream);
 
+/*
+ * bltc_gi_update_noalloc -- bltc_gi_update for callers that must not allocate device memory.
+ *
+ * Who needs it: callers for whom cudaMalloc / cudaMallocAsync is off limits or bound to fail at the point where
+ * they call us.  Examples: a solver embedded in a host application that handed all of HBM to its own arena at
+ * start-up, so the driver has nothing left to give; a plug-in whose host forbids driver allocations inside its
+ * callbacks; a process that runs under a fixed device-memory budget it may not exceed once initialised; a
+ * latency-bound inner loop (one such update follows each of the 188-1246 convolutions of an SCF step,
+ * PAPER.md:311,338) that cannot accept the implicit synchronisation or the milliseconds an allocation may cost.
+ * bltc_gi_update itself takes the block partial sums of its reductions from the library's stream-ordered pool on
+ * every call; this variant keeps them in a fixed array inside the library image instead.
+ *
+ * Same arithmetic, same kernels, same grid and summation order as bltc_gi_update (Algorithm 2 lines 4-7,
+ * PAPER.md:127-133, Eq. (27)): on the same device buffers the two give the same result.  Arguments and
+ * the layout of `result` are those of bltc_gi_update, with these differences:
+ *   - EVERY buffer (w, psi_old, f_old, psi_new, phi, result) must be device (or managed) memory, owned by the
+ *     caller; a host pointer is refused with BLTC_EINVAL, because staging it would need an allocation;
+ *   - n_prev <= BLTC_GI_NOALLOC_MAX_PREV (64); a larger n_prev is refused with BLTC_EINVAL and a message naming
+ *     the limit (use bltc_gi_update then).  N is not limited beyond bltc_gi_update's [1, 2e9];
+ *   - the call makes no cudaMalloc, cudaFree, cudaMallocAsync or other allocating call, ever; it only enqueues
+ *     4 kernels on `stream` and returns without synchronising.
+ * Cost: the array is 139,264 doubles = 1.06 MiB of device memory on every GPU that loads libbltc.so, held from
+ * library load until the process exits, whether or not this entry point is ever called.
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress, with that device current)
+ * and the SM count, once, and remembers them.  Make that first call outside any stream capture -- e.g. one warm-up
+ * call per device at start-up.
+ * Sharing: all calls on one GPU use the SAME array.  It needs no clearing between calls (every slot a call reads
+ * was written earlier in that same call), but two calls whose kernels can overlap on the GPU -- different streams,
+ * different host threads, without an ordering between them -- race on it and both results are garbage.  Serialise
+ * them on one stream or with events.  bltc_gi_update (pool scratch per call) has no such restriction.
+ */
+#define BLTC_GI_NOALLOC_MAX_PREV 64
+int bltc_gi_update_noalloc(const double* w, const double* psi_old, const double* f_old, double* psi_new,
+                           const double* phi, int n_prev, int64_t N, double eps_old, double* result,
+                           bltc_stream stream);
+
 int bltc_destroy(bltc_handle h);
 
 int bltc_get_stats(bltc_handle h, bltc_stats* s);

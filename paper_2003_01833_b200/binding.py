@@ -47,7 +47,7 @@ EXPORTED = ("bltc_create", "bltc_create_host_plan", "bltc_create_sharded", "bltc
             "bltc_create_with_builder",
             "bltc_get_shard_targets", "bltc_convolve", "direct_convolve", "bltc_convolve_scatter",
             "bltc_convolve_coulomb_scatter",
-            "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_destroy",
+            "bltc_convolve_coulomb", "direct_convolve_coulomb", "bltc_gi_update", "bltc_gi_update_noalloc", "bltc_destroy",
             "bltc_get_stats", "bltc_export_plan", "bltc_export_proxy", "bltc_set_profiling",
             "bltc_get_phase_ms", "bltc_direct_set_profiling", "bltc_direct_get_kernel_ms",
             "bltc_probe_fp64", "bltc_probe_fp64_form", "bltc_orbital_tiles", "bltc_last_error", "bltc_version")
@@ -79,6 +79,7 @@ def lib():
     L.direct_convolve_coulomb.argtypes = [vp, vp, C.c_int64, vp, vp, vp, C.c_int64, C.c_int, vp, C.c_int,
                                           C.c_double, vp]
     L.bltc_gi_update.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int64, C.c_double, vp, vp]
+    L.bltc_gi_update_noalloc.argtypes = L.bltc_gi_update.argtypes
     L.bltc_destroy.argtypes = [vp]
     L.bltc_get_stats.argtypes = [vp, C.POINTER(bltc_stats)]
     L.bltc_export_plan.argtypes = [vp, _i64p, _i64p, _i64p, _i64p, _dp, _dp, _i32p, _i32p, _i64p, _i64p,
@@ -292,6 +293,25 @@ def bltc_gi_update(w, psi_old, f_old, psi_new, phi, n_prev, N, eps_old, result, 
     _check(lib().bltc_gi_update(_ptr(w, "w", False, N), _ptr(psi_old, "psi_old", False, N), _ptr(f_old, "f_old", False, N),
                                 _ptr(psi_new, "psi_new", False, N), _ptr(phi, "phi", True, n_prev * N), n_prev, N,
                                 float(eps_old), _ptr(result, "result", False, 4 + n_prev), _stream_ptr(stream)))
+    return result
+
+
+GI_NOALLOC_MAX_PREV = 64      # BLTC_GI_NOALLOC_MAX_PREV of include/bltc.h
+
+
+def bltc_gi_update_noalloc(w, psi_old, f_old, psi_new, phi, n_prev, N, eps_old, result, stream=None):
+    """include/bltc.h bltc_gi_update_noalloc: bltc_gi_update for callers that cannot allocate device memory (an
+    application whose own arena already owns all of HBM, a host that forbids driver allocations in its callbacks, a
+    fixed memory budget, a loop that cannot afford an allocation's synchronisation).  The reduction scratch is a
+    1.06 MiB array inside libbltc.so instead of pool memory, so: every buffer must be a CUDA tensor,
+    n_prev <= GI_NOALLOC_MAX_PREV (64), and two calls that may overlap on one GPU race on that array -- keep them on
+    one stream.  The first call on a device looks up the array's address; make it before any stream capture.
+    This wrapper allocates nothing either: it passes the addresses of the caller's tensors."""
+    N, n_prev = int(N), int(n_prev)
+    _check(lib().bltc_gi_update_noalloc(
+        _ptr(w, "w", False, N), _ptr(psi_old, "psi_old", False, N), _ptr(f_old, "f_old", False, N),
+        _ptr(psi_new, "psi_new", False, N), _ptr(phi, "phi", True, n_prev * N), n_prev, N,
+        float(eps_old), _ptr(result, "result", False, 4 + n_prev), _stream_ptr(stream)))
     return result
 
 

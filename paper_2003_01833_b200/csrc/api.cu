@@ -926,6 +926,10 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
 
 }  // namespace
 
+namespace bltc {
+int set_last_error(int code, const char* msg) { return fail(code, msg ? msg : ""); }
+}  // namespace bltc
+
 extern "C" {
 
 int direct_convolve(const double* targets, const double* f_targets, int64_t M,

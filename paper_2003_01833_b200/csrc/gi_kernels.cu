@@ -15,8 +15,12 @@
 // consumer in the same fixed pattern) => bitwise reproducible, no atomics.  The consumer kernel's prologue finishes the
 // producer's reduction, so no extra launch or host round trip sits between the steps.
 #include <cuda_runtime.h>
+#include <cmath>
 #include <cstdint>
+#include <mutex>
+#include <string>
 
+#include "../../include/bltc.h"
 #include "gi_kernels.cuh"
 
 namespace bltc {
@@ -188,3 +192,110 @@ cudaError_t launch_gi_update(const double* w, const double* psi_old, const doubl
 size_t gi_scratch_doubles(int n_prev, int nblk) { return (size_t)nblk * (2 + n_prev) + 2 * (size_t)nblk; }
 
 }  // namespace bltc
+
+// ---------------------------------------------------------------------------------------------------------------
+// bltc_gi_update_noalloc (include/bltc.h): the same four kernels as bltc_gi_update, for callers that are not allowed
+// to allocate device memory.  bltc_gi_update takes the block partial sums of its two-level reductions from the
+// library's stream-ordered pool (cudaMallocFromPoolAsync); here they live in the fixed array below, which is part of
+// the library image: the driver reserves it on every GPU that loads libbltc.so and keeps it until the process exits.
+//
+// Size: kGiNoallocMaxBlocks x (2 + kGiNoallocMaxPrev) doubles for the dot products + 2 x kGiNoallocMaxBlocks for the
+// norm and the residual = 139,264 doubles = 1.06 MiB per GPU.
+//
+// Nothing in the array has to start at zero: each of the three reductions writes every slot it later reads (one slot
+// per block and quantity, all blocks of the fixed grid), so what the previous call left behind is never read and no
+// clearing pass is needed.  What the shared array does cost is concurrency: two calls in flight on the same GPU at
+// the same time (two streams, two host threads, two graphs) write the same slots and corrupt each other's sums.
+namespace {
+
+constexpr int kGiNoallocMaxPrev = BLTC_GI_NOALLOC_MAX_PREV;
+constexpr int kGiNoallocMaxBlocks = 2048;
+constexpr size_t kGiNoallocDoubles =
+    (size_t)kGiNoallocMaxBlocks * (2 + kGiNoallocMaxPrev) + 2 * (size_t)kGiNoallocMaxBlocks;
+
+static __device__ __align__(256) double g_gi_noalloc_scratch[kGiNoallocDoubles];
+
+constexpr int kMaxDevices = 64;
+
+struct GiNoallocDevice {
+    double* scratch = nullptr;       // DEVICE address of g_gi_noalloc_scratch on this GPU
+    int nblk_cap = 0;                // SM count x 8, at most kGiNoallocMaxBlocks
+};
+
+// Per-GPU set-up, done by the first call on each device with that device current.  In host code the name
+// g_gi_noalloc_scratch is only the handle the runtime registered for the symbol; the address a kernel can
+// dereference differs per GPU and has to be asked for.  cudaGetSymbolAddress may initialise the context and load the
+// module, which is why the first call on a device belongs before any stream capture.
+cudaError_t gi_noalloc_device(GiNoallocDevice* out) {
+    static std::mutex mu;
+    static GiNoallocDevice table[kMaxDevices];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!table[dev].scratch) {
+        double* ptr = nullptr;
+        e = cudaGetSymbolAddress((void**)&ptr, g_gi_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        const int cap = (sms > 0 ? sms : 148) * 8;
+        table[dev].nblk_cap = cap < kGiNoallocMaxBlocks ? cap : kGiNoallocMaxBlocks;
+        table[dev].scratch = ptr;
+    }
+    *out = table[dev];
+    return cudaSuccess;
+}
+
+bool gi_noalloc_on_device(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" int bltc_gi_update_noalloc(const double* w, const double* psi_old, const double* f_old, double* psi_new,
+                                      const double* phi, int n_prev, int64_t N, double eps_old, double* result,
+                                      bltc_stream stream) {
+    using bltc::set_last_error;
+    // argument and size checks first: they need no device, and a refused call must not touch the shared array
+    if (!w || !psi_old || !f_old || !psi_new || !result) return set_last_error(BLTC_EINVAL, "NULL argument");
+    if (N < 1 || N > 2000000000LL) return set_last_error(BLTC_EINVAL, "N must be in [1, 2e9]");
+    if (n_prev < 0) return set_last_error(BLTC_EINVAL, "n_prev must be >= 0");
+    if (n_prev > kGiNoallocMaxPrev)
+        return set_last_error(BLTC_EINVAL,
+                              ("bltc_gi_update_noalloc: n_prev = " + std::to_string(n_prev) +
+                               " exceeds BLTC_GI_NOALLOC_MAX_PREV = " + std::to_string(kGiNoallocMaxPrev) +
+                               ", the most the library's fixed scratch array holds; use bltc_gi_update").c_str());
+    if (n_prev > 0 && !phi) return set_last_error(BLTC_EINVAL, "phi is NULL but n_prev > 0");
+    if (!std::isfinite(eps_old)) return set_last_error(BLTC_EINVAL, "eps_old must be finite");
+    // host buffers would need a staging copy on the device, i.e. an allocation: refused here
+    if (!gi_noalloc_on_device(w) || !gi_noalloc_on_device(psi_old) || !gi_noalloc_on_device(f_old) ||
+        !gi_noalloc_on_device(psi_new) || !gi_noalloc_on_device(result) || (n_prev > 0 && !gi_noalloc_on_device(phi)))
+        return set_last_error(BLTC_EINVAL,
+                              "bltc_gi_update_noalloc: every buffer must be device memory (staging a host buffer "
+                              "would allocate); use bltc_gi_update for host buffers");
+    GiNoallocDevice d;
+    cudaError_t e = gi_noalloc_device(&d);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return set_last_error(BLTC_ECUDA, (std::string("bltc_gi_update_noalloc set-up (cudaGetSymbolAddress): ") +
+                                           cudaGetErrorString(e)).c_str());
+    }
+    // the grid of bltc_gi_update (gi_grid_blocks), so that both entry points sum in the same order
+    const int64_t need = (N + bltc::kGiThreads - 1) / bltc::kGiThreads;
+    const int nblk = (int)(need < d.nblk_cap ? need : d.nblk_cap);
+    if (bltc::gi_scratch_doubles(n_prev, nblk) > kGiNoallocDoubles)       // cannot happen given the two caps above
+        return set_last_error(BLTC_EINVAL, "bltc_gi_update_noalloc: scratch array too small");
+    e = bltc::launch_gi_update(w, psi_old, f_old, psi_new, phi, n_prev, N, eps_old, result, d.scratch, nblk,
+                               static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return set_last_error(BLTC_ECUDA, (std::string("bltc_gi_update_noalloc launch: ") + cudaGetErrorString(e)).c_str());
+    }
+    return BLTC_OK;
+}

@@ -8,6 +8,9 @@ namespace bltc {
 // layout of the result vector of bltc_gi_update (include/bltc.h)
 enum { kGiEpsNew = 0, kGiDelta = 1, kGiNorm = 2, kGiResidual = 3, kGiCoeff = 4 };
 
+// records `msg` as the calling thread's bltc_last_error() and returns `code` (defined in api.cu)
+int set_last_error(int code, const char* msg);
+
 int gi_grid_blocks(int64_t n, int sm_count);
 size_t gi_scratch_doubles(int n_prev, int nblk);
 
