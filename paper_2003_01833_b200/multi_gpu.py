@@ -129,6 +129,9 @@ class ShardedPlan:
 
     def _run(self, call_plain, call_scatter, n_orb, out, gather):
         if not self.fused:
+            if out is None:                  # `out` is optional in both modes: the plain path needs a buffer of its own
+                import torch
+                out = torch.empty((n_orb, self.N), dtype=torch.float64, device=self.device)
             call_plain(out)
             return self.exchange.all_gather_out(out) if gather else out
         t, hdl, peers = self._symm_out(n_orb)
