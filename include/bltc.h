@@ -200,9 +200,10 @@ int bltc_convolve_coulomb_scatter(bltc_handle h, const double* f, int n_f, doubl
  *   sources double[3][N], weights double[N], f_sources double[n_orb][N], k HOST double[n_orb],
  *   out double[n_orb][M].
  * The call synchronises `stream` once before the pair kernel is enqueued: the bounding boxes of target and
- * source chunks are read back to choose the kernel variant (r == 0 test only where a source chunk can meet a
- * target chunk, exp underflow guard only if k_max x the largest distance can reach 700).  Its profiling switch
- * (bltc_direct_set_profiling) is per calling thread.
+ * source chunks are read back to choose the kernel variant (exp underflow guard only if k_max x the largest
+ * distance can reach 700).  Every pair goes through the r == 0 test: the kernel runs the one loop that skips
+ * coincident points everywhere (it costs no FP64 instruction; a second loop without it was slower).  Its
+ * profiling switch (bltc_direct_set_profiling) is per calling thread.
  */
 int direct_convolve(const double* targets, const double* f_targets, int64_t M,
                     const double* sources, const double* weights, const double* f_sources, int64_t N,

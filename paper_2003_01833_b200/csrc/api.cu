@@ -805,9 +805,9 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
         nsplit = (int)std::min<int64_t>(nsplit, std::max<int64_t>(1, N / 256));
     }
     // Bounding boxes of the pseudo-batches and of the source segments (one small kernel each, read back: the one
-    // synchronisation of this call).  A segment whose box does not meet the batch's box cannot hold a source that
-    // coincides with one of its targets, so its tiles run without the r == 0 test (reading R3); and the exp
-    // underflow guard is compiled in only if k_max x (the largest possible distance) can reach 700.
+    // synchronisation of this call): the exp underflow guard is compiled in only if k_max x (the largest possible
+    // distance) can reach 700.  The r == 0 test (reading R3) runs for every pair: launch_near below is called with
+    // all_zero_safe = true, which ignores Range::flags, so no per-range "may coincide" flag is computed here.
     const int64_t seg_len = std::max<int64_t>(1, (N + nsplit - 1) / nsplit);
     const int nseg_box = (int)((N + seg_len - 1) / seg_len);
     std::vector<double> box_t((size_t)npb64 * 6), box_s((size_t)nseg_box * 6);
@@ -844,13 +844,7 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
             pb_base.push_back((int64_t)nsplit * b0);
             for (int s = 0; s < nsplit; ++s) {
                 const int64_t s0 = std::min<int64_t>(N, (int64_t)s * seg_len), s1 = std::min<int64_t>(N, (int64_t)(s + 1) * seg_len);
-                bool touch = s1 > s0;
-                if (touch) {
-                    const int sb = (int)(s0 / seg_len);
-                    for (int d = 0; d < 3; ++d)
-                        touch = touch && box_s[sb * 6 + d] <= box_t[pb * 6 + 3 + d] && box_t[pb * 6 + d] <= box_s[sb * 6 + 3 + d];
-                }
-                ranges.push_back(Range{(int32_t)s0, (int32_t)s1, touch ? kRangeMayCoincide : 0});
+                ranges.push_back(Range{(int32_t)s0, (int32_t)s1, kRangeMayCoincide});
             }
         }
         const int unit = 32 * kTargetsPerThread;
@@ -928,6 +922,12 @@ int direct_impl(int kind, const double* targets, const double* f_targets, int64_
 
 namespace bltc {
 int set_last_error(int code, const char* msg) { return fail(code, msg ? msg : ""); }
+
+cudaError_t pool_alloc_async(void** p, size_t bytes, cudaStream_t st) {
+    cudaMemPool_t pool = TempBuf::library_pool();
+    if (!pool) return cudaMallocAsync(p, bytes ? bytes : 1, st);
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, st);
+}
 }  // namespace bltc
 
 extern "C" {
