@@ -14,7 +14,7 @@
 //          rho = u - rint(u) in [-1/2, 1/2];   exp(-k r) = 2^n * 2^(j/T) * (1 + rho (C1 + C2 rho))
 //          2^(j/T): 64 KB shared-memory table per CTA, read by per-lane LDS.64 (random entries: ~4.4 SM cycles
 //          per warp lookup against 2 conflict-free, measured; a 16-copy conflict-free table of 512 entries needs
-//          the cubic polynomial again and was measured slower, profiles/r02a_variants.md);
+//          the cubic polynomial again and was measured slower, tuning log);
 //          2^n: the table's high words are pre-biased by -(j << 7), so adding (m << 7) -- one shift, one add,
 //          both on the ALU pipe -- puts the biased exponent n + 1023 and the mantissa of 2^(j/T) in place.
 //          6 FP64 instructions per exp.  Quadratic near-minimax polynomial: relative error <= 6.3e-15 (about 28

@@ -1,4 +1,5 @@
-"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs, every element
+of every output entering the norm below (one test, ..._elementwise_without_cancellation, bounds each element by itself).
 
 Tolerances (BASELINE.json north_star; norm per DESIGN.md R13: unweighted relative 2-norm per orbital,
 max over orbitals):
@@ -120,6 +121,38 @@ def test_direct_large_k_r_underflow_is_harmless(gpu, oracle_mod):
     ref = oracle_mod.direct(P, P, c.w, c.f, c.k, f_tgt=c.f)
     got = gpu_direct(gpu, c)
     assert np.all(np.isfinite(got)) and rel2(got, ref) <= TOL_DIRECT
+
+
+def test_direct_few_dominant_neighbours_elementwise_without_cancellation(gpu, oracle_mod):
+    """Worst case for the 6-instruction exp (quadratic polynomial, per-evaluation error <= 6.3e-15 relative, DESIGN.md
+    section 7): the other direct tests pass on a relative 2-NORM over sums of thousands of terms of either sign, where
+    the polynomial's error averages out.  Here nothing averages: f > 0 and w > 0 (every term has the same sign, no
+    subtraction), a handful of sources, and k so large that one or two nearest neighbours make up a target's whole sum
+    -- each output carries the error of a single kernel evaluation, and EVERY ELEMENT has to meet the bound.
+    Bound per element: 6.3e-15 (exp) + a few ulp (rsqrt, products) + the conditioning of exp(-k r) on r, which neither
+    side can avoid: |d exp(-kr)| / exp(-kr) = k r |dr| / r, with |dr| / r of an ulp or two on either side."""
+    rng = np.random.default_rng(20030183 + 515)
+    Ns, M = 12, 3000
+    c = I.random_cloud(Ns, n_orb=3, seed=41)
+    c.w = rng.random(Ns) + 0.1
+    c.f = np.ascontiguousarray(rng.random((3, Ns)) + 0.05)
+    c.k = np.array([0.7, 9.0, 40.0])
+    S = c.coords()
+    lo, hi = S.min(axis=1, keepdims=True), S.max(axis=1, keepdims=True)
+    T = np.ascontiguousarray(lo + (hi - lo) * rng.random((3, M)))
+    rmax = float(np.linalg.norm(hi - lo))
+    torch, B = gpu
+    out = torch.empty((3, M), dtype=torch.float64, device="cuda")
+    B.direct_convolve(dev(torch, T), None, M, dev(torch, S), dev(torch, c.w), dev(torch, c.f), Ns, c.k, 3, out, False)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    ref = oracle_mod.direct((T[0], T[1], T[2]), (c.x, c.y, c.z), c.w, c.f, c.k, subtract=False)
+    assert np.all(ref < 0.0)                                             # -2 x a sum of positive terms: no cancellation
+    err = np.abs(got - ref) / np.abs(ref)
+    for o in range(3):
+        bound = 1.0e-14 + 4.5e-16 * c.k[o] * rmax
+        print(f"k = {c.k[o]}: max element-wise relative error {err[o].max():.2e} (bound {bound:.2e})")
+        assert err[o].max() <= bound, (o, err[o].max(), bound)
 
 
 def test_direct_config1_sampled(gpu, oracle_mod):

@@ -97,7 +97,7 @@ def check_full_size(gpu, oracle_mod, c, batches, orbitals, subtract, n_direct=60
 @pytest.mark.parametrize("theta,degree,tol", [(0.8, 6, 1e-3), (0.6, 8, 5e-6), (0.6, 6, 2e-4), (0.8, 8, 5e-5), (0.7, 8, 2e-5)])
 def test_config2_co_like(gpu, oracle_mod, theta, degree, tol):
     # BASELINE.json configs[2]: theta in {0.6, 0.8} x degree in {6, 8} -- all four -- plus the paper's (0.7, 8) at
-    # which north_star states its 1e-6 method target; 7 orbitals = register tiles 4 + 3
+    # which north_star states its 1e-6 method target; 7 orbitals = one register tile of 7
     c = I.config2(theta=theta, degree=degree)
     check_full_size(gpu, oracle_mod, c, batches=[3, 611], orbitals=[0, 3, 4, 6], subtract=True, tol_method=tol)
 
@@ -116,7 +116,7 @@ def test_config2_error_decreases_with_degree_and_smaller_theta(gpu):
 
 
 def test_config3_c6h6_like(gpu, oracle_mod):
-    # BASELINE.json configs[3]: 3.46 M points, 21 orbitals (register tiles 4,4,4,3,3,3), theta 0.7, degree 8
+    # BASELINE.json configs[3]: 3.46 M points, 21 orbitals (register tiles 7,7,7), theta 0.7, degree 8
     c = I.config3()
     check_full_size(gpu, oracle_mod, c, batches=[17, 4242], orbitals=[0, 7, 13, 20], subtract=True,
                     n_direct=300, n_cpu_direct=24, tol_method=5e-6)
