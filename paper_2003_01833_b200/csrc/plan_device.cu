@@ -36,11 +36,19 @@ constexpr double kSqrt2 = 1.4142135623730951;
         if (e__ != cudaSuccess) return e__;                 \
     } while (0)
 
+// Temporary of one plan build, from the library's stream-ordered pool (a cudaMalloc / cudaFree pair per temporary
+// made bltc_create depend on the host and the driver's state: GPUTEST_r02 read 48 ms for the lists stage on one box
+// and 5 ms on another).  The builders run on ONE stream, given once per thread before the first alloc.
+thread_local cudaStream_t t_scratch_stream = nullptr;
 template <typename T>
 struct Scratch {
     T* p = nullptr;
-    ~Scratch() { if (p) cudaFree(p); }
-    cudaError_t alloc(size_t n) { return cudaMalloc(&p, (n ? n : 1) * sizeof(T)); }
+    ~Scratch() { release(); }
+    void release() { if (p) cudaFreeAsync(p, t_scratch_stream); p = nullptr; }
+    cudaError_t alloc(size_t n) {
+        release();
+        return pool_alloc_async(reinterpret_cast<void**>(&p), (n ? n : 1) * sizeof(T), t_scratch_stream);
+    }
 };
 
 // order-preserving map double -> uint64 (exact for min/max by integer atomics)
@@ -139,6 +147,7 @@ ord_kernel(const int32_t* __restrict__ seg_begin, int nseg, int64_t n, int32_t* 
 cudaError_t build_tree_device(Tree& t, const double* d_coords, int64_t n, int64_t max_leaf, int32_t* d_perm,
                               cudaStream_t st) {
     if (n >= (int64_t)1 << 28) return cudaErrorInvalidValue;      // keys are segment << 3 in 32 bits
+    t_scratch_stream = st;
     t.cl.clear(); t.perm.clear(); t.leaves.clear();
     const unsigned grid = (unsigned)((n + 255) / 256);
     Scratch<uint32_t> key0, key1, run_key;
@@ -153,9 +162,6 @@ cudaError_t build_tree_device(Tree& t, const double* d_coords, int64_t n, int64_
     auto ensure_seg = [&](size_t need) -> cudaError_t {
         if (need <= seg_cap) return cudaSuccess;
         seg_cap = std::max(need, 2 * seg_cap + 1024);
-        for (auto* s : {&box_slot, &seg_begin}) { if (s->p) cudaFree(s->p); s->p = nullptr; }
-        if (lo.p) cudaFree(lo.p); if (hi.p) cudaFree(hi.p); if (split.p) cudaFree(split.p);
-        lo.p = hi.p = nullptr; split.p = nullptr;
         BLTC_DEV_TRY(box_slot.alloc(seg_cap)); BLTC_DEV_TRY(seg_begin.alloc(seg_cap));
         BLTC_DEV_TRY(lo.alloc(3 * seg_cap)); BLTC_DEV_TRY(hi.alloc(3 * seg_cap)); BLTC_DEV_TRY(split.alloc(seg_cap));
         return cudaSuccess;
@@ -238,13 +244,18 @@ cudaError_t build_tree_device(Tree& t, const double* d_coords, int64_t n, int64_
         cur = dv.Current() == vals[0] ? 0 : 1;
         tb = temp_bytes;
         BLTC_DEV_TRY(cub::DeviceRunLengthEncode::Encode(temp.p, tb, dk.Current(), run_key.p, run_cnt.p, num_runs.p, (int)n, st));
+        // one read-back per level: the run count together with the runs themselves.  A segment yields at most 8 runs
+        // (its child codes) and there are no more runs than points, so the copy is sized by that bound instead of
+        // waiting for the count first (that cost a second host round trip per tree level).
         int32_t nr = 0;
+        const size_t run_cap = (size_t)std::min<int64_t>(n, 8 * (int64_t)ns);
+        h_key.resize(run_cap); h_cnt.resize(run_cap);
         BLTC_DEV_TRY(cudaMemcpyAsync(&nr, num_runs.p, sizeof nr, cudaMemcpyDeviceToHost, st));
+        BLTC_DEV_TRY(cudaMemcpyAsync(h_key.data(), run_key.p, run_cap * 4, cudaMemcpyDeviceToHost, st));
+        BLTC_DEV_TRY(cudaMemcpyAsync(h_cnt.data(), run_cnt.p, run_cap * 4, cudaMemcpyDeviceToHost, st));
         BLTC_DEV_TRY(cudaStreamSynchronize(st));
+        if (nr < 0 || (size_t)nr > run_cap) return cudaErrorUnknown;
         h_key.resize(nr); h_cnt.resize(nr);
-        BLTC_DEV_TRY(cudaMemcpyAsync(h_key.data(), run_key.p, (size_t)nr * 4, cudaMemcpyDeviceToHost, st));
-        BLTC_DEV_TRY(cudaMemcpyAsync(h_cnt.data(), run_cnt.p, (size_t)nr * 4, cudaMemcpyDeviceToHost, st));
-        BLTC_DEV_TRY(cudaStreamSynchronize(st));
         // next level's segments = the runs; the runs of an active segment are its children in code order
         std::vector<Seg> next;
         next.reserve(nr);
@@ -361,6 +372,7 @@ inline double half_diag(const double* lo, const double* hi) {
 
 cudaError_t build_lists_device(HostPlan& p, int shard_rank, int shard_world, cudaStream_t st) {
     const int ncl = (int)p.src.cl.size(), nb = (int)p.b_begin.size();
+    t_scratch_stream = st;
     std::vector<MacCluster> hc(ncl);
     {   // skip pointers: the cluster after c's subtree in pre-order
         std::vector<int> last(ncl);

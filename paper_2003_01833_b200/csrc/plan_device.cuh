@@ -7,6 +7,10 @@
 
 namespace bltc {
 
+// Stream-ordered scratch from the library's own per-device memory pool (api.cu): after the first bltc_create the
+// two dozen temporaries of a plan build are served from memory the pool kept, not by cudaMalloc / cudaFree.
+cudaError_t pool_alloc_async(void** p, size_t bytes, cudaStream_t st);
+
 // Builds the cluster tree of the n points d_coords (device, SoA double[3][n]) with leaves of <= max_leaf points:
 // t.cl (DFS pre-order, boxes, ranges, parents, children) and t.leaves on the host, the tree-order -> caller-index
 // permutation in d_perm (device int32[n]); t.perm stays empty.  Identical to build_tree() of plan_host.cpp.
