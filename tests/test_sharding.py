@@ -271,9 +271,77 @@ def test_gpu_sharded_plan_with_nccl_world1_equals_plain_convolve():
         B.bltc_convolve(plan, c.k, f, c.n_orb, ref)
         torch.cuda.synchronize()
         assert torch.equal(out, ref)
+        got = sp.convolve(c.k, f, c.n_orb)            # `out` left out: the plain path allocates the result itself
+        torch.cuda.synchronize()
+        assert got.data_ptr() != out.data_ptr() and torch.equal(got, ref)
         sp.destroy(); B.bltc_destroy(plan)
     finally:
         dist.destroy_process_group()
+
+
+def _cuda_world2_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2003_01833_b200.multi_gpu import ShardExchange
+        torch.cuda.set_device(0)                                  # both ranks share the one GPU there is
+        c = I.random_cloud(6000, n_orb=3, seed=22, clustered=True, leaf_size=200, batch_size=200, degree=4)
+        X = torch.from_numpy(c.coords()).cuda(); w = torch.from_numpy(c.w).cuda()
+        f = torch.from_numpy(np.ascontiguousarray(c.f)).cuda()
+        plan = B.bltc_create_sharded(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size, rank, world)
+        st = B.bltc_get_stats(plan)
+        idx = B.bltc_get_shard_targets(plan)
+        out = torch.full((c.n_orb, c.N), float("nan"), dtype=torch.float64, device="cuda")
+        B.bltc_convolve(plan, c.k, f, c.n_orb, out, True)         # this rank's CUDA kernels, its slice of the batches only
+        torch.cuda.synchronize()
+        mine = out.cpu()
+        written = ~torch.isnan(mine[0])
+        only_own = bool(np.array_equal(np.sort(torch.nonzero(written)[:, 0].numpy()), np.sort(idx)))
+        ex = ShardExchange(idx, c.N, "cpu")                       # the exchange: values over gloo, no GPU rank waits on another
+        ex.all_gather_out(mine)
+        evals = torch.tensor([st["shard_far_evals"] + st["shard_near_evals"], int(only_own), len(idx)], dtype=torch.int64)
+        dist.all_reduce(evals, op=dist.ReduceOp.SUM)
+        if rank == 0:
+            full = B.bltc_create(None, X, w, c.N, c.theta, c.degree, c.batch_size, c.leaf_size)
+            ref = torch.empty_like(out)
+            B.bltc_convolve(full, c.k, f, c.n_orb, ref, True)
+            torch.cuda.synchronize()
+            fs = B.bltc_get_stats(full)
+            q.put((mine.numpy(), ref.cpu().numpy(), [int(v) for v in evals], fs["far_evals"] + fs["near_evals"]))
+            B.bltc_destroy(full)
+        B.bltc_destroy(plan)
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_gpu_world2_sharded_cuda_path_two_processes_on_one_gpu(oracle_mod):
+    """The N > 1 path with the CUDA kernels in it, as far as one GPU allows: two processes, both on cuda:0, each builds
+    its bltc_create_sharded(rank, 2) plan and runs bltc_convolve for its slice; the slices are exchanged as CPU tensors
+    by ShardExchange over gloo (no kernel of one rank waits on the other's).  The assembled result must be BITWISE the
+    unsharded GPU result (the slice's work items and summation order are the full plan's) and within 1e-12 of the oracle."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_cuda_world2_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got, ref, sums, full_evals = q.get(timeout=600)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    c = I.random_cloud(6000, n_orb=3, seed=22, clustered=True, leaf_size=200, batch_size=200, degree=4)
+    assert sums[0] == full_evals and sums[1] == 2 and sums[2] == c.N     # the slices partition work and targets
+    assert not np.isnan(got).any()
+    np.testing.assert_array_equal(got, ref)
+    op = oracle_mod.OraclePlan((c.x, c.y, c.z), c.theta, c.degree, c.leaf_size, c.batch_size)
+    want = op.evaluate(c.w, c.f, c.k)
+    err = max(np.linalg.norm(got[o] - want[o]) / np.linalg.norm(want[o]) for o in range(c.n_orb))
+    assert err <= 1e-12, err
 
 
 @pytest.mark.gpu
