@@ -131,7 +131,8 @@ class ClockSampler:
 
 
 def workload(name="cfg1", kernel="yukawa", orbitals=0):
-    """cfg1 (BASELINE.json configs[1]) is the bench workload; the others are for profiling and context runs.
+    """cfg3 (BASELINE.json configs[3], the largest single-GPU config) is the bench workload; cfg1 rides along as a
+    5-step context run, the others are for profiling.
     kernel = "coulomb": the same mesh with ONE field, the density rho = 2 sum_o psi_o^2 -- the Hartree
     potential of bltc_convolve_coulomb (Table 4's workload shape)."""
     from paper_2003_01833_b200 import inputs as I
@@ -151,13 +152,17 @@ def sample_batches(n_batches, count=4):
     return sorted(set(int(round(i * (n_batches - 1) / max(count - 1, 1))) for i in range(count)))
 
 
-CPU_SAMPLE_BATCHES = 4      # both CPU legs (cpu_baseline inside the CUDA arm, --impl reference) time this sample
+# Both CPU legs (cpu_baseline inside the CUDA arm, --impl reference) time this sample.  40 and not 4: with 4 batches the
+# batch-sum phase ran 0.14-0.19 s and carried 97 % of the extrapolated time, so two runs of the same oracle on the same
+# box differed by 24 % (BENCH_r02); 40 batches give it ~2 s on configs[3] while the proxy-charge phase barely grows
+# (a few batches already need the charges of most clusters).
+CPU_SAMPLE_BATCHES = 40
 
 
 _ORACLE_PLANS = {}
 
 
-def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
+def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False, n_batches=None):
     """Time the CPU oracle's BLTC (as it stands) on a bounded sample of the workload -- CPU_SAMPLE_BATCHES evenly
     spread target batches, the first orbital -- and scale to the whole convolution phase by phase: the proxy-charge
     phase (Alg. 3 line 2) by particle-cluster pairs, the batch-cluster sums (line 3) by kernel evaluations, both times
@@ -173,7 +178,7 @@ def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
         _ORACLE_PLANS[key] = (op, op.export())
     op, e = _ORACLE_PLANS[key]
     size = e["cl_end"] - e["cl_begin"]
-    batches = sample_batches(op.n_batches, CPU_SAMPLE_BATCHES)
+    batches = sample_batches(op.n_batches, n_batches or CPU_SAMPLE_BATCHES)
     ev, need = 0, set()
     for b in batches:
         nt = e["b_end"][b] - e["b_begin"][b]
@@ -204,6 +209,7 @@ def cpu_oracle_sample(c, repeat=1, kernel="yukawa", fast=False):
             f"({ntg} targets) x 1 of {c.n_orb} orbitals, {threads} OpenMP threads over clusters / targets: "
             f"{t_up:.2f} s proxy charges ({up_sample:.3g} of {up_total:.3g} particle-cluster pairs) + {t_ev:.2f} s "
             f"batch sums ({ev:.3g} of {ev_total:.3g} kernel evaluations); each phase scaled by its count, x n_orb")
+    cpu_oracle_sample.last_phase_s = {"proxy_charges": t_up, "batch_sums": t_ev}
     return value, dt, desc, threads
 
 
@@ -243,7 +249,8 @@ def run_reference(args):
         "dtype": "f64", "data": "synthetic",
         "config": config_dict(c, args, args.gpus),
         "note": "each step = the CPU oracle on a bounded sample of the workload (see cpu_baseline.sample)",
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "phase_s": cpu_oracle_sample.last_phase_s},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -253,7 +260,7 @@ def run_reference(args):
 
 # FP64 instructions per (target, source / proxy point) pair of a tile of ot orbitals, as (first orbital, each further one),
 # counted in the SASS (python -m paper_2003_01833_b200.sass_count), and how many of them are DFMAs with three distinct
-# vector-register sources -- those hold the FP64 pipe for 3 cycles instead of 2 on sm_100a (profiles/r02h_probes.md)
+# vector-register sources -- those hold the FP64 pipe for 3 cycles instead of 2 on sm_100a (microbenchmark table; this run's own dfma_probe_tflops)
 FP64_INSTR_PER_PAIR = {"near": (22.0, 9.0), "far": (17.0, 9.0), "far9": (148.0 / 9, 9.0)}
 FP64_3REG_PER_PAIR = {"near": 1.0, "far": 2.0, "far9": 2.0}            # per orbital: the accumulate (+ fhat - f_i what)
 
@@ -293,7 +300,8 @@ def roofline_of(phase_ms, st, groups, degree, coulomb, probe, steps, sm_mhz=None
 
 def committed_traffic(workload_name, kernel):
     """DRAM bytes of one launch of `kernel` on this workload from the committed ncu capture (profiles/r02_traffic.csv:
-    workload,kernel,dram_bytes_per_launch -- profiles/r02_traffic.md names the command); None if not captured."""
+    workload,kernel,dram_bytes_per_launch -- profiles/r02h_cfg3_launches.md names the command); None if not captured.
+    A CONSTANT read from that file, not measured in this run: the line says so in roofline.traffic_source."""
     tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     try:
         for line in open(tpath):
@@ -370,6 +378,16 @@ def run_cuda(args):
             plan = B.bltc_create(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size)
             create_ms = (time.perf_counter() - t0) * 1e3
         st = B.bltc_get_stats(plan)
+        host_builder = None
+        if not shard:                                    # the threaded host builder on the same box, for comparison
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            hplan = B.bltc_create_with_builder(None, X, w, N, c.theta, c.degree, c.batch_size, c.leaf_size, 0, 1,
+                                               B.BUILDER_HOST)
+            hms = (time.perf_counter() - t0) * 1e3
+            hst = B.bltc_get_stats(hplan)
+            host_builder = {"create_ms": hms, "build_ms": hst["build_ms"], "upload_ms": hst["upload_ms"]}
+            B.bltc_destroy(hplan)
 
         def convolve(f_, out_):
             if fused is not None:                        # epilogue scatters over NVLink peer memory (symmetric memory)
@@ -449,7 +467,7 @@ def run_cuda(args):
             same = bool(torch.equal(res.cpu(), out.cpu()))
             e2e = {"ms_per_step": e2e_ms, "steps": e2e_steps, "bitwise_equal_to_device_path": same}
         return dict(plan=plan, st=st, X=X, w=w, f=f, out=out, ms_per_step=ms_per_step, phase_sum=phase_sum,
-                    create_ms=create_ms, create_cold_ms=create_cold_ms, clocks=clocks, e2e=e2e)
+                    create_ms=create_ms, create_cold_ms=create_cold_ms, host_builder=host_builder, clocks=clocks, e2e=e2e)
 
     # ---- the headline workload ----------------------------------------------------------------
     c = workload(args.workload, args.kernel, args.orbitals)
@@ -526,6 +544,7 @@ def run_cuda(args):
             if rank == 0 else None)
     phase_ms = {p: v / args.steps for p, v in R["phase_sum"].items()}
     create_ms, create_cold_ms, clocks, e2e_info = R["create_ms"], R["create_cold_ms"], R["clocks"], R["e2e"]
+    host_builder = R["host_builder"]
     B.bltc_destroy(plan)
     del X, w, f, out, R
 
@@ -547,7 +566,11 @@ def run_cuda(args):
         dom = "near" if roof["near"]["ms_per_step"] >= roof["far"]["ms_per_step"] else "far"
         other = "far" if dom == "near" else "near"
         roof[dom]["traffic"] = committed_traffic(args.workload if not args.orbitals else "", dom + "_kernel")
+        roof[dom]["traffic_source"] = (None if roof[dom]["traffic"] is None else
+                                       "committed ncu capture of an earlier build, not this run: profiles/r02_traffic.csv "
+                                       "(command in profiles/r02h_cfg3_launches.md)")
         cpu_v, cpu_dt, cpu_desc, cores = cpu_oracle_sample(c, kernel=args.kernel)
+        cpu_phase_s = cpu_oracle_sample.last_phase_s
         fast_v, fast_dt, fast_desc, fast_cores = cpu_oracle_sample(c, kernel=args.kernel, fast=True)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -558,7 +581,10 @@ def run_cuda(args):
             "actual_evals_per_s": (st["near_evals"] + st["far_evals"]) * O * jobs / (ms_per_step * 1e-3),
             "phase_ms": phase_ms,
             "plan": {"create_ms": create_ms, "create_cold_ms": create_cold_ms,
-                     "host_build_ms": st["build_ms"], "upload_ms": st["upload_ms"],
+                     "built_on_device": bool(st["built_on_device"]), "build_ms": st["build_ms"],
+                     "stage_ms": {"tree": st["tree_ms"], "lists": st["lists_ms"], "decomposition": st["decomp_ms"],
+                                  "upload_and_proxy_weights": st["upload_ms"]},
+                     "host_builder": host_builder,
                      "clusters": st["n_clusters"], "batches": st["n_batches"],
                      "far_evals": st["far_evals"], "near_evals": st["near_evals"]},
             "roofline": roof[dom], "roofline_" + other: roof[other],
@@ -574,7 +600,8 @@ def run_cuda(args):
             "cfg1": cfg1,
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks,
-            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc,
+                             "phase_s": cpu_phase_s},
             "cpu_baseline_fast": {"value": fast_v, "unit": UNIT, "cores": fast_cores, "kind": "oracle, fast-math build",
                                   "sample": fast_desc},
         }

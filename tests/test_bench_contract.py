@@ -46,7 +46,7 @@ def test_cpu_baseline_sample_uses_every_thread():
     ncpu = os.cpu_count() or 1
     if ncpu < 4:
         pytest.skip("needs >= 4 cores")
-    code = ("import bench, json; c = bench.workload('cfg0'); v, dt, desc, cores = bench.cpu_oracle_sample(c, repeat=2); "
+    code = ("import bench, json; c = bench.workload('cfg0'); v, dt, desc, cores = bench.cpu_oracle_sample(c, repeat=2, n_batches=4); "
             "print(json.dumps({'dt': dt, 'cores': cores, 'value': v}))")
     res = {}
     for nt in (1, 4):
