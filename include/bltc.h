@@ -32,7 +32,9 @@
  *   - Return value: 0 on success, a negative bltc_status otherwise; bltc_last_error() gives a
  *     thread-local message.  No exceptions, no exit(); handles are independent and the library keeps no state
  *     between calls other than a stream-ordered memory pool of its own per device (staging buffers of
- *     direct_convolve / bltc_gi_update are reused, the device's default pool is not touched).
+ *     direct_convolve / bltc_gi_update and the temporaries of bltc_create are reused, the device's default pool is
+ *     not touched), the fixed scratch array of bltc_gi_update_noalloc, and the per-thread profiling switch of
+ *     direct_convolve.  It reads one environment variable, BLTC_ORBITAL_TILE (see "Diagnostics" below).
  *     A handle must not be used by two threads at once.  Calls on one handle share its scratch (proxy charges,
  *     partial sums, staging); the library orders them itself: a convolve enqueued on another stream than the
  *     previous one first waits (cudaStreamWaitEvent) for that one to finish.
@@ -324,6 +326,17 @@ int bltc_export_plan(bltc_handle h, int64_t* src_perm, int64_t* tgt_perm,
 int bltc_export_proxy(bltc_handle h, int32_t* proxy_cluster, double* nodes, double* what,
                       double* fhat, int32_t* ot);
 
+/*
+ * ---------------------------------------------------------------------------------------------------------------
+ * Diagnostics.  Everything from here to bltc_orbital_tiles serves measurement (bench.py, the tuning runs behind
+ * DESIGN.md 10) and is not needed to compute a convolution: per-phase and per-kernel timers, the DFMA-rate probes
+ * behind the roofline denominator, and the orbital-tile query.
+ * One environment variable belongs here too, the only one the library reads: BLTC_ORBITAL_TILE = 1 .. 7 caps the
+ * width of the orbital register tile (tuning runs and the tile-width tests); it is read by every bltc_convolve /
+ * direct_convolve / bltc_orbital_tiles call, so it may be changed between calls.  Unset, the library chooses the
+ * widths itself (bltc_orbital_tiles).  Results at different widths agree to rounding, not bitwise.
+ * ---------------------------------------------------------------------------------------------------------------
+ */
 /* Per-phase device timing.  enable = 1: every later bltc_convolve records CUDA events on its stream
  * around each phase.  bltc_get_phase_ms synchronises on the last recorded event and returns the
  * milliseconds of each phase of the most recent convolve, summed over its orbital groups. */
